@@ -1,0 +1,430 @@
+#!/usr/bin/env python
+"""bench.py -- PLIC solves per second on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--log2n 26]
+
+Workload (config.workload): BASELINE.json configs[1] -- N = 2^26 cells, fp32 SoA, seed 1,
+normals uniform on the unit sphere, V0 ~ U[0,1) (gen.random_sphere).  1.07 GB in + 0.27 GB
+out per launch, far larger than the 126 MB L2, so consecutive steps cannot hit in cache.
+
+A step is one plic_solve launch over the whole batch: load, mirror/sort, volume reduction,
+case selection, per-case solve, sign restore, store with one
+method.  All eight method variants and plic_volume (row a7) are timed the same way in the
+same run (W warm-up + K timed launches each, CUDA events on the launching stream) and listed
+under "methods"; the headline `value` is the fastest variant that the parity tests hold to
+the 2e-5 bound -- all of them are, see tests/test_parity_gpu.py -- named in config.method.
+
+Multi-GPU (torchrun, one rank per GPU): the path has no exchange step, so rank r solves its
+own 2^26 cells [r 2^26, (r+1) 2^26) of the same seeded stream, no data-path collective;
+`value` = all ranks' cells / max-over-ranks time ("scaling": "weak").
+
+--impl reference times the fp64 CPU oracle (oracle/), as it stands, on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "plic_solves_per_second"
+UNIT = "Gcells/s"
+BYTES_PER_CELL = 20                      # 4 fp32 read + 1 fp32 written
+WORKLOAD = "configs[1]: N=2^%d cells, fp32 SoA, seed 1, normals uniform on sphere, V0~U[0,1)"
+SEED = 1
+FALLBACK_HBM_GBS = 6650.0                # B200_PROFILING.md fallback
+
+
+# ------------------------------------------------------------------------------------------
+# distributed helpers (also exercised on CPU with gloo by tests/test_shard_gloo.py)
+# ------------------------------------------------------------------------------------------
+def rank_cells(per_rank: int, rank: int):
+    """Weak scaling: rank r owns cells [r*per_rank, (r+1)*per_rank) of the seeded stream."""
+    return rank * per_rank, (rank + 1) * per_rank
+
+
+def _dist():
+    import torch.distributed as dist
+    return dist if dist.is_available() and dist.is_initialized() else None
+
+
+def max_over_ranks(x: float, device="cuda") -> float:
+    dist = _dist()
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(x: float, device="cuda") -> float:
+    dist = _dist()
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def barrier():
+    dist = _dist()
+    if dist is not None:
+        dist.barrier()
+
+
+# ------------------------------------------------------------------------------------------
+# clocks: NVML sampled from a thread during the timed regions
+# ------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown",
+               0x4: "sw_power_cap", 0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting"}
+
+    def __init__(self, torch_device_index: int, period_s: float = 0.004):
+        self.samples = []          # (t, sm_mhz, reasons bitmask, power W)
+        self.period = period_s
+        self.ok = False
+        self.sm_max = None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            uuid = str(torch.cuda.get_device_properties(torch_device_index).uuid)
+            if not uuid.startswith("GPU-"):
+                uuid = "GPU-" + uuid
+            try:
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode())
+            except Exception:
+                vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+                idx = int(vis.split(",")[torch_device_index]) if vis and vis.split(",")[0].isdigit() \
+                    else torch_device_index
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(idx)
+            self.sm_max = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:      # noqa: BLE001
+            self.err = repr(e)
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                sm = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                try:
+                    rs = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    rs = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                try:
+                    pw = nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+                except Exception:
+                    pw = None
+                self.samples.append((time.perf_counter(), int(sm), int(rs), pw))
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def start(self):
+        if self.ok:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join(timeout=2.0)
+
+    def summary(self, windows):
+        """Median SM clock and the union of event reasons over samples inside `windows`
+        (list of (t0, t1) perf_counter intervals = the timed regions)."""
+        if not self.ok:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0,
+                    "note": "NVML unavailable: %s" % getattr(self, "err", "?")}
+        ins = [s for s in self.samples if any(a <= s[0] <= b for a, b in windows)]
+        note = "NVML samples inside the timed regions"
+        if len(ins) < 3:           # regions shorter than the sampling period: widen to the phase
+            lo = min(a for a, _ in windows) - 0.05
+            hi = max(b for _, b in windows) + 0.05
+            ins = [s for s in self.samples if lo <= s[0] <= hi]
+            note = "NVML samples over the whole timing phase (regions shorter than the sampler period)"
+        if not ins:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": [], "samples": 0, "note": note}
+        clocks = sorted(s[1] for s in ins)
+        mask = 0
+        for s in ins:
+            mask |= s[2]
+        reasons = [name for bit, name in self.REASONS.items() if mask & bit]
+        pw = [s[3] for s in ins if s[3] is not None]
+        return {"sm_mhz": clocks[len(clocks) // 2], "sm_min_mhz": clocks[0], "sm_max_mhz": self.sm_max,
+                "reasons": reasons, "samples": len(ins), "power_w_max": max(pw) if pw else None,
+                "note": note}
+
+
+# ------------------------------------------------------------------------------------------
+# the oracle leg (cpu_baseline and --impl reference)
+# ------------------------------------------------------------------------------------------
+def oracle_rate(arrays, n_cells: int):
+    """Times oracle.solve on the first n_cells of the workload; returns (cells/s, seconds)."""
+    import oracle
+    sub = [a[:n_cells] for a in arrays]
+    t0 = time.perf_counter()
+    oracle.solve(*sub)
+    dt = time.perf_counter() - t0
+    return n_cells / dt, dt
+
+
+def cpu_baseline(arrays, budget_s: float = 12.0):
+    import oracle
+    N = arrays[0].shape[0]
+    cal = min(N, 1 << 20)
+    rate, _ = oracle_rate(arrays, cal)                       # calibration (also warms the .so)
+    n = int(min(N, max(cal, rate * budget_s)))
+    rate, dt = oracle_rate(arrays, n)
+    return {"value": rate / 1e9, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+            "sample": "first %d cells of the workload (%.1f s of fp64 bisection, all host threads)" % (n, dt)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import gen
+    import oracle
+    N = 1 << args.log2n
+    cal_n = 1 << 20
+    arrays = gen.random_sphere(min(N, 1 << 24), SEED)
+    rate, _ = oracle_rate(arrays, cal_n)
+    # each step: a bounded sample so that (K + W) steps end within ~2 minutes
+    per_step_s = max(0.25, min(4.0, 120.0 / max(1, args.steps + args.warmup)))
+    n = int(min(arrays[0].shape[0], max(cal_n, rate * per_step_s)))
+    for _ in range(args.warmup):
+        oracle_rate(arrays, n)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_rate(arrays, n)
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt / 1e9
+    sample = "each step = oracle.solve on the first %d cells of the workload" % n
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": WORKLOAD % args.log2n, "method": "oracle: fp64 forward map + bisection",
+                   "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs: torch copy, best of 10)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md, MEASURED_PEAKS.json absent)"
+
+
+def ncu_traffic(kernel_name: str):
+    """dram bytes per launch of `kernel_name` from the committed ncu summary, or None."""
+    p = os.path.join(ROOT, "profiles", "dram_traffic.txt")
+    try:
+        with open(p) as f:
+            for line in f:
+                parts = line.split()
+                if len(parts) >= 2 and parts[0] == kernel_name:
+                    return float(parts[1])
+    except Exception:
+        pass
+    return None
+
+
+def time_launches(fn, steps, warmup, stream):
+    """W untimed + K timed calls of fn() on `stream`; barrier + synchronize on both sides;
+    device time from CUDA events recorded on that stream.  Returns (ms total, (t0, t1) host window)."""
+    import torch
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    barrier()
+    torch.cuda.synchronize()
+    e0 = torch.cuda.Event(enable_timing=True)
+    e1 = torch.cuda.Event(enable_timing=True)
+    w0 = time.perf_counter()
+    e0.record(stream)
+    for _ in range(steps):
+        fn()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    barrier()
+    torch.cuda.synchronize()
+    w1 = time.perf_counter()
+    return e0.elapsed_time(e1), (w0, w1)
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import gen
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- libplic has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import paper_2006_12838_b200 as plic           # raises if libplic.so cannot be built/loaded
+
+    N = 1 << args.log2n
+    lo, hi = rank_cells(N, rank)
+    host = gen.random_sphere(N, SEED, start=lo)                       # fp32 V0, nx, ny, nz
+    dV, dx, dy, dz = [torch.from_numpy(a).cuda() for a in host]
+    out = torch.empty_like(dV)
+    stream = torch.cuda.current_stream()
+
+    variants = [(m, f) for f in (True, False) for m in ("analytic", "sz", "newton", "nested")]
+    sampler = ClockSampler(local)
+    sampler.start()
+
+    # bring the clocks up before any timing (not counted as warm-up steps)
+    t_end = time.perf_counter() + args.prewarm_ms / 1e3
+    while time.perf_counter() < t_end:
+        for _ in range(20):
+            plic.plic_solve(dV, dx, dy, dz, out=out, method="analytic", fast=True)
+        torch.cuda.synchronize()
+
+    methods = {}
+    windows = {}
+    launches_before = plic.plic_launch_count()
+    for m, f in variants:
+        name = plic.plic_method_name(plic.method_id(m, f))
+        c0 = plic.plic_launch_count()
+        ms, win = time_launches(lambda: plic.plic_solve(dV, dx, dy, dz, out=out, method=m, fast=f),
+                                args.steps, args.warmup, stream)
+        timed_launches = (plic.plic_launch_count() - c0) - args.warmup
+        ms = max_over_ranks(ms)
+        grid, block, cpt = plic.plic_launch_config(m, N, f)
+        gcs = N * world * args.steps / (ms * 1e-3) / 1e9
+        methods[name] = {"value": gcs, "ms_per_step": ms / args.steps, "launches": timed_launches,
+                         "hbm_gbs_per_gpu": BYTES_PER_CELL * N * args.steps / (ms * 1e-3) / 1e9,
+                         "grid": grid, "block": block}
+        windows[name] = win
+    vol = torch.empty_like(dV)
+    ms, win = time_launches(lambda: plic.plic_volume(out, dx, dy, dz, out=vol),
+                            args.steps, args.warmup, stream)
+    ms = max_over_ranks(ms)
+    methods["plic_volume"] = {"value": N * world * args.steps / (ms * 1e-3) / 1e9,
+                              "ms_per_step": ms / args.steps, "launches": args.steps,
+                              "hbm_gbs_per_gpu": BYTES_PER_CELL * N * args.steps / (ms * 1e-3) / 1e9}
+    windows["plic_volume"] = win
+    total_launches = plic.plic_launch_count() - launches_before
+
+    solve_names = [plic.plic_method_name(plic.method_id(m, f)) for m, f in variants]
+    head = args.method if args.method != "auto" else max(solve_names, key=lambda k: methods[k]["value"])
+    H = methods[head]
+    peak, peak_src = measured_peak()
+    for k, v in methods.items():
+        v["roofline_frac"] = v["hbm_gbs_per_gpu"] / peak
+
+    # ---- end to end through the host-array C ABI: pinned host buffers, copies inside ----------
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    pin = [torch.from_numpy(a).pin_memory() for a in host]
+    pout = torch.empty(N, dtype=torch.float32).pin_memory()
+    hm, hf = (head[:-5], True) if head.endswith("-fast") else (head, False)
+    for _ in range(2):
+        plic.plic_solve_host(*pin, out=pout, method=hm, fast=hf)
+    torch.cuda.synchronize()
+    barrier()
+    c0 = plic.plic_launch_count()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        plic.plic_solve_host(*pin, out=pout, method=hm, fast=hf)      # synchronous
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    e2e_launches = plic.plic_launch_count() - c0
+    e2e_s = max_over_ranks(t1 - t0)
+    plic.plic_solve(dV, dx, dy, dz, out=out, method=hm, fast=hf)
+    e2e_same = bool(np.array_equal(pout.numpy(), out.cpu().numpy()))   # host API == device API, bitwise
+    sampler.stop()
+    plic.plic_host_release()
+
+    clocks = sampler.summary([windows[head]])
+    if rank == 0:
+        traffic = ncu_traffic(head)
+        achieved = H["hbm_gbs_per_gpu"]
+        line = {
+            "metric": METRIC, "value": H["value"], "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": H["ms_per_step"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": WORKLOAD % args.log2n, "cells_per_gpu": N, "method": head,
+                       "headline_rule": "fastest of the 8 plic_solve variants" if args.method == "auto"
+                       else "--method",
+                       "l2": "inputs larger than L2 (1.07 GB read + 0.27 GB written per step vs 126 MB)",
+                       "prewarm_ms": args.prewarm_ms, "launch": {"grid": H["grid"], "block": H["block"],
+                                                                 "cells_per_thread": 4}},
+            "clocks": clocks,
+            "gpu_launches": H["launches"],
+            "gpu_launches_all_timed_regions": total_launches,
+            "e2e": {"value": N * world * e2e_steps / e2e_s / 1e9, "unit": UNIT,
+                    "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 4 * N, "steps": e2e_steps,
+                    "launches": e2e_launches, "matches_device_api_bitwise": e2e_same, "api": "plic_solve_host (pinned host arrays, chunked "
+                    "H2D/kernel/D2H pipeline inside libplic)", "timer": "host wall clock around the "
+                    "synchronous calls, device synchronised on both sides"},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": traffic, "kernel": head,
+                         "algorithmic_bytes_per_launch": BYTES_PER_CELL * N, "peak_source": peak_src},
+            "methods": methods,
+        }
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = cpu_baseline(host)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--log2n", type=int, default=26, help="cells per GPU = 2^log2n (default: configs[1])")
+    ap.add_argument("--method", default="auto", help="headline variant, e.g. analytic-fast (default: fastest)")
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--prewarm-ms", type=float, default=300.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args(argv)
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                       # timing rule: at least 3 warm-up steps
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

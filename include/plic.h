@@ -1,0 +1,133 @@
+/*
+ * plic.h -- C ABI of libplic: the batched PLIC plane-cube problem on one B200 (sm_100a).
+ *
+ * PAPER.md below is /root/reference/PAPER.md, the text of arxiv 2006.12838 ("Analytic
+ * Solution to the Piecewise Linear Interface Construction Problem ...").
+ *
+ * The operation (eq. (1)): for each of N independent cells, a truncated
+ * volume V0 in [0,1] and a plane normal n = (nx,ny,nz) are mapped to the plane offset
+ *
+ *     d0 in [-S/2, +S/2],  S = |nx|+|ny|+|nz|,
+ *
+ * such that the half-space { x : n.x <= d0 } cuts the volume V0 out of the unit cube
+ * [-1/2,1/2]^3 (plic_solve).  plic_volume is the forward map V0(d0, n) of PAPER.md:71-92,
+ * eq. (6), (7), (11).  Every step -- mirror/sort (eq. (2)-(4)), volume reduction (eq. (5)),
+ * case selection (eq. (26)), the per-case solve (eq. (25), sect. 2.4, 2.5) and the sign
+ * restore (eq. (8)) -- runs in hand-written CUDA kernels; there is no CPU fallback.
+ *
+ * Data layout: structure of arrays, five flat fp32 arrays of N elements each.
+ * Algorithmic HBM traffic is 20 B per cell (16 B read, 4 B written).
+ */
+#ifndef PLIC_H_
+#define PLIC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Same opaque type as the CUDA runtime's cudaStream_t (a redeclaration of an identical
+ * typedef is legal C11/C++), so this header needs no CUDA include. */
+typedef struct CUstream_st *cudaStream_t;
+
+/* ---- method ids: `method` = one of PLIC_METHOD_* optionally OR-ed with PLIC_FAST ---------- */
+#define PLIC_METHOD_ANALYTIC 0 /* the paper's analytic inverse: eq. (12), (14)-(26), Listing 2
+                                   */
+#define PLIC_METHOD_SZ       1 /* Scardovelli-Zaleski solution, edge-case complete and
+                                  micro-optimised: sect. 2.4, Listings 3/4 */
+#define PLIC_METHOD_NEWTON   2 /* Newton-Raphson for cases (1),(3),(4): sect. 2.5, Listing 6
+                                   */
+#define PLIC_METHOD_NESTED   3 /* nested intervals (bisection) for cases (3),(4): sect. 2.5,
+                                  Listing 5 */
+#define PLIC_NUM_METHODS     4
+#define PLIC_FAST        0x100 /* approximate SFU roots/reciprocals/trig and branch-free,
+                                  a-priori case selection; without it: IEEE division and
+                                  square root, CUDA libm cbrt/asin/acos/sin/cos */
+
+/* ---- error codes (functions return 0 on success, never throw, never print) ---------------- */
+#define PLIC_OK               0
+#define PLIC_ERR_NULL        -1 /* a null pointer with N > 0 */
+#define PLIC_ERR_SIZE        -2 /* N < 0 */
+#define PLIC_ERR_METHOD      -3 /* unknown method id */
+#define PLIC_ERR_LAUNCH      -4 /* the CUDA runtime reported an error (launch, copy, alloc) */
+#define PLIC_ERR_ALIGN       -5 /* a pointer is not 4-byte aligned */
+
+/*
+ * plic_solve -- d0[i] = d0(V0[i], n[i]) for i in [0, N)            (eq. (1))
+ *
+ *   V0, nx, ny, nz  DEVICE pointers, fp32, N elements each, read only.
+ *   d0              DEVICE pointer, fp32, N elements, written.  May be the same pointer as
+ *                   V0 (each cell is read and then written by the same thread); any other
+ *                   overlap is undefined.
+ *   N               number of cells, >= 0.  N == 0 is a successful no-op.
+ *   method          PLIC_METHOD_* [| PLIC_FAST].
+ *   stream          the CUDA stream the work is enqueued on (0 = legacy default stream).
+ *
+ * The caller owns all memory.  The call allocates nothing, keeps no per-call state, does
+ * not synchronise and returns as soon as the kernels are enqueued.  Pointers need only be
+ * 4-byte aligned: when all five share one alignment modulo 16 the body runs on 128-bit
+ * loads/stores and at most 3 head + 3 tail cells take a scalar kernel; otherwise the whole
+ * range takes the scalar kernel (correct, slower).
+ *
+ * Input domain (paper: V0 in [0,1], |n|_2 = 1).  Outside it: V0 < 0 acts as 0, V0 > 1 as 1;
+ * n need not be normalised exactly -- every method is written so that
+ * d0(V0, c n) = c d0(V0, n) up to rounding; n = (0,0,0) gives d0 = 0.  For every finite
+ * input the result is finite (no NaN), including n1 = 0, n1 = n2 = 0 and V0 in {0, 1/2, 1}
+ * (PAPER.md:155-181, 217).  A NaN input gives an unspecified finite or NaN output.
+ *
+ * Returns PLIC_OK or a negative PLIC_ERR_*.
+ */
+int plic_solve(const float *V0, const float *nx, const float *ny, const float *nz,
+               float *d0, int64_t N, int method, cudaStream_t stream);
+
+/*
+ * plic_volume -- V0[i] = V0(d0[i], n[i]): the forward map ("inverse PLIC", Listing 1,
+ * PAPER.md:71-92; eq. (2)-(4), (7), (11), (6)).  Same argument conventions as plic_solve
+ * with d0 read and V0 written (V0 may be the same pointer as d0).  |d0| > S/2 (plane misses
+ * the cube) gives 0 or 1.  n = (0,0,0) gives 0, 1/2, 1 for d0 <, =, > 0.
+ */
+int plic_volume(const float *d0, const float *nx, const float *ny, const float *nz,
+                float *V0, int64_t N, cudaStream_t stream);
+
+/*
+ * plic_solve_host / plic_volume_host -- the same maps for HOST arrays (pageable or pinned;
+ * pinned memory makes the copies asynchronous).  The range is cut into chunks; host->device
+ * copies, the kernel and the device->host copy of consecutive chunks overlap on three
+ * internal streams of the current device.  Synchronous: the result is complete in d0 / V0
+ * when the call returns.  A device workspace (3 x 5 x chunk fp32) is allocated on first use
+ * per device, kept for later calls and freed by plic_host_release().  Not re-entrant: calls
+ * from several host threads are serialised by an internal lock.
+ */
+int plic_solve_host(const float *V0, const float *nx, const float *ny, const float *nz,
+                    float *d0, int64_t N, int method);
+int plic_volume_host(const float *d0, const float *nx, const float *ny, const float *nz,
+                     float *V0, int64_t N);
+/* Frees the host-API workspace and streams of every device; safe to call at any time. */
+void plic_host_release(void);
+
+/* "analytic", "sz", "newton", "nested" (+ "-fast" with PLIC_FAST); NULL if unknown.
+ * The string is static storage owned by the library. */
+const char *plic_method_name(int method);
+
+/* Static text for a PLIC_ERR_* code (never NULL). */
+const char *plic_error_string(int code);
+
+/* ABI version: 100*major + minor. */
+int plic_version(void);
+
+/*
+ * plic_launch_config -- the launch geometry plic_solve (method >= 0) or plic_volume
+ * (method == -1) uses for N cells with 16-byte aligned pointers on the current device:
+ * *grid thread blocks of *block threads, each thread handling *cells_per_thread cells per
+ * grid-stride step.  For reporting only.  Returns PLIC_OK or an error code.
+ */
+int plic_launch_config(int method, int64_t N, int *grid, int *block, int *cells_per_thread);
+
+/* Number of kernels this library has launched in this process since load (all threads). */
+int64_t plic_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PLIC_H_ */

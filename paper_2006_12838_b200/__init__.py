@@ -1,0 +1,216 @@
+"""paper_2006_12838_b200 -- Python binding of libplic (include/plic.h): argument marshalling only.
+
+Every step of the PLIC path (mirror/sort, volume reduction, case selection, the per-case
+solve, sign restore; eq. (1)-(8), (11), (25), (26)) runs in the CUDA kernels of
+``csrc/``.  This module loads ``libplic.so`` with ctypes, passes raw device (or host)
+pointers, sizes and the CUDA stream handle, and turns error codes into exceptions.  PyTorch
+appears only as the owner of device memory and streams.  There is no CPU fallback: if the
+shared library is missing it is built with nvcc, and if that fails the import raises.
+
+    plic_solve(V0, nx, ny, nz, out=None, method="analytic", fast=False, stream=None) -> d0
+    plic_volume(d0, nx, ny, nz, out=None, stream=None) -> V0
+    plic_solve_host / plic_volume_host      same maps for host arrays (numpy or CPU tensors)
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+from . import build as _build
+
+__all__ = ["METHODS", "FAST", "method_id", "plic_solve", "plic_volume", "plic_solve_host",
+           "plic_volume_host", "plic_host_release", "plic_method_name", "plic_error_string",
+           "plic_version", "plic_launch_config", "plic_launch_count", "PlicError", "lib",
+           "LIB_PATH"]
+
+METHODS = {"analytic": 0, "sz": 1, "newton": 2, "nested": 3}
+FAST = 0x100
+LIB_PATH = _build.LIB
+
+
+class PlicError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        super().__init__("%s failed: %s (code %d)" % (what, plic_error_string(code), code))
+        self.code = code
+
+
+def _load() -> ctypes.CDLL:
+    path = _build.build()          # no-op when libplic.so is newer than its sources
+    lib_ = ctypes.CDLL(path)
+    fp = ctypes.c_void_p
+    i64 = ctypes.c_int64
+    ip = ctypes.POINTER(ctypes.c_int)
+    lib_.plic_solve.argtypes = [fp, fp, fp, fp, fp, i64, ctypes.c_int, ctypes.c_void_p]
+    lib_.plic_solve.restype = ctypes.c_int
+    lib_.plic_volume.argtypes = [fp, fp, fp, fp, fp, i64, ctypes.c_void_p]
+    lib_.plic_volume.restype = ctypes.c_int
+    lib_.plic_solve_host.argtypes = [fp, fp, fp, fp, fp, i64, ctypes.c_int]
+    lib_.plic_solve_host.restype = ctypes.c_int
+    lib_.plic_volume_host.argtypes = [fp, fp, fp, fp, fp, i64]
+    lib_.plic_volume_host.restype = ctypes.c_int
+    lib_.plic_host_release.argtypes = []
+    lib_.plic_host_release.restype = None
+    lib_.plic_method_name.argtypes = [ctypes.c_int]
+    lib_.plic_method_name.restype = ctypes.c_char_p
+    lib_.plic_error_string.argtypes = [ctypes.c_int]
+    lib_.plic_error_string.restype = ctypes.c_char_p
+    lib_.plic_version.argtypes = []
+    lib_.plic_version.restype = ctypes.c_int
+    lib_.plic_launch_config.argtypes = [ctypes.c_int, i64, ip, ip, ip]
+    lib_.plic_launch_config.restype = ctypes.c_int
+    lib_.plic_launch_count.argtypes = []
+    lib_.plic_launch_count.restype = i64
+    return lib_
+
+
+lib = _load()
+
+
+def method_id(method, fast: bool = False) -> int:
+    """'analytic' | 'sz' | 'newton' | 'nested' (optionally with a '-fast' suffix) or an int id."""
+    if isinstance(method, str):
+        name = method
+        if name.endswith("-fast"):
+            name, fast = name[:-5], True
+        if name not in METHODS:
+            raise ValueError("unknown PLIC method %r" % (method,))
+        mid = METHODS[name]
+    else:
+        mid = int(method)
+    return mid | (FAST if fast else 0)
+
+
+def plic_method_name(method: int):
+    s = lib.plic_method_name(int(method))
+    return s.decode() if s is not None else None
+
+
+def plic_error_string(code: int) -> str:
+    return lib.plic_error_string(int(code)).decode()
+
+
+def plic_version() -> int:
+    return int(lib.plic_version())
+
+
+def plic_launch_count() -> int:
+    return int(lib.plic_launch_count())
+
+
+def plic_launch_config(method, N: int, fast: bool = False):
+    """(grid, block, cells_per_thread) of plic_solve (method id/name) or plic_volume (method=-1)."""
+    g, b, c = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+    mid = -1 if method == -1 else method_id(method, fast)
+    rc = lib.plic_launch_config(mid, int(N), ctypes.byref(g), ctypes.byref(b), ctypes.byref(c))
+    if rc != 0:
+        raise PlicError(rc, "plic_launch_config")
+    return g.value, b.value, c.value
+
+
+def plic_host_release() -> None:
+    lib.plic_host_release()
+
+
+# ------------------------------------------------------------------------------------------
+# device-pointer API (torch CUDA tensors)
+# ------------------------------------------------------------------------------------------
+def _device_args(first, nx, ny, nz, out):
+    import torch
+    N = first.numel()
+    for t in (first, nx, ny, nz):
+        if not (t.is_cuda and t.dtype == torch.float32 and t.dim() == 1 and t.is_contiguous()
+                and t.numel() == N and t.device == first.device):
+            raise ValueError("inputs must be contiguous 1-D float32 CUDA tensors of one length "
+                             "on one device")
+    if out is None:
+        out = torch.empty_like(first)
+    elif not (out.is_cuda and out.dtype == torch.float32 and out.is_contiguous()
+              and out.numel() == N and out.device == first.device):
+        raise ValueError("out must be a contiguous float32 CUDA tensor of the inputs' length")
+    return N, out
+
+
+def _stream_handle(stream, device):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream(device)
+    return ctypes.c_void_p(int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def plic_solve(V0, nx, ny, nz, out=None, method="analytic", fast: bool = False, stream=None):
+    """d0 = d0(V0, n) per cell (eq. (1)) on the tensors' device; returns `out`."""
+    import torch
+    N, out = _device_args(V0, nx, ny, nz, out)
+    with torch.cuda.device(V0.device):
+        rc = lib.plic_solve(V0.data_ptr(), nx.data_ptr(), ny.data_ptr(), nz.data_ptr(),
+                            out.data_ptr(), N, method_id(method, fast),
+                            _stream_handle(stream, V0.device))
+    if rc != 0:
+        raise PlicError(rc, "plic_solve")
+    return out
+
+
+def plic_volume(d0, nx, ny, nz, out=None, stream=None):
+    """V0 = V0(d0, n) per cell (eq. (6), (7), (11)) on the tensors' device; returns `out`."""
+    import torch
+    N, out = _device_args(d0, nx, ny, nz, out)
+    with torch.cuda.device(d0.device):
+        rc = lib.plic_volume(d0.data_ptr(), nx.data_ptr(), ny.data_ptr(), nz.data_ptr(),
+                             out.data_ptr(), N, _stream_handle(stream, d0.device))
+    if rc != 0:
+        raise PlicError(rc, "plic_volume")
+    return out
+
+
+# ------------------------------------------------------------------------------------------
+# host-pointer API (numpy arrays or CPU torch tensors, pinned or pageable)
+# ------------------------------------------------------------------------------------------
+def _host_ptr(a, N=None):
+    import numpy as np
+    if hasattr(a, "data_ptr"):                       # CPU torch tensor
+        import torch
+        if a.is_cuda or a.dtype != torch.float32 or not a.is_contiguous() or a.dim() != 1:
+            raise ValueError("host arrays must be contiguous 1-D float32 CPU tensors")
+        n, p = a.numel(), a.data_ptr()
+    else:
+        if not (isinstance(a, np.ndarray) and a.dtype == np.float32 and a.ndim == 1
+                and a.flags.c_contiguous):
+            raise ValueError("host arrays must be contiguous 1-D float32 numpy arrays")
+        n, p = a.shape[0], a.ctypes.data
+    if N is not None and n != N:
+        raise ValueError("host arrays must have one length")
+    return n, p
+
+
+def _host_out(first, out):
+    import numpy as np
+    if out is not None:
+        return out
+    if hasattr(first, "data_ptr"):
+        import torch
+        return torch.empty_like(first)
+    return np.empty_like(first)
+
+
+def plic_solve_host(V0, nx, ny, nz, out=None, method="analytic", fast: bool = False):
+    """plic_solve for host arrays: chunked H2D / kernel / D2H pipeline inside libplic."""
+    N, p0 = _host_ptr(V0)
+    ptrs = [p0] + [_host_ptr(a, N)[1] for a in (nx, ny, nz)]
+    out = _host_out(V0, out)
+    ptrs.append(_host_ptr(out, N)[1])
+    rc = lib.plic_solve_host(*ptrs, N, method_id(method, fast))
+    if rc != 0:
+        raise PlicError(rc, "plic_solve_host")
+    return out
+
+
+def plic_volume_host(d0, nx, ny, nz, out=None):
+    """plic_volume for host arrays."""
+    N, p0 = _host_ptr(d0)
+    ptrs = [p0] + [_host_ptr(a, N)[1] for a in (nx, ny, nz)]
+    out = _host_out(d0, out)
+    ptrs.append(_host_ptr(out, N)[1])
+    rc = lib.plic_volume_host(*ptrs, N)
+    if rc != 0:
+        raise PlicError(rc, "plic_volume_host")
+    return out

@@ -1,0 +1,357 @@
+// plic_kernels.cu -- kernels, launch logic and the C ABI of libplic (include/plic.h).
+//
+// One elementwise pass per call: 16 B read + 4 B written per cell, no reuse, so the kernels
+// are built around HBM streaming: 128-bit loads of four SoA arrays (one float4 = 4 cells per
+// array per thread), L1 no-allocate, a persistent grid of (SM count x resident blocks)
+// thread blocks striding over the array, 128-bit stores.  Not a contraction: no tensor
+// cores, no shared-memory staging (each byte is used exactly once by exactly one thread).
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <atomic>
+#include <mutex>
+
+#include "../../include/plic.h"
+#include "plic_methods.cuh"
+
+#define PLIC_VERSION 100
+
+namespace plic {
+
+constexpr int kBlock = 256;        // threads per block
+constexpr int kMaxDevices = 64;
+
+__device__ __forceinline__ float4 ld_stream(const float4 *p) {
+    float4 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                 : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void st_stream(float4 *p, const float4 &v) {
+    asm volatile("st.global.cs.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(v.x), "f"(v.y),
+                 "f"(v.z), "f"(v.w)
+                 : "memory");
+}
+
+// op(V0-or-d0, nx, ny, nz) -> result, for one cell
+template <int METHOD, bool FAST>
+struct SolveOp {
+    static __device__ __forceinline__ float apply(float s, float x, float y, float z) {
+        return solve_cell<METHOD, FAST>(s, x, y, z);
+    }
+};
+struct VolumeOp {
+    static __device__ __forceinline__ float apply(float s, float x, float y, float z) {
+        return volume_cell(s, x, y, z);
+    }
+};
+
+// Body: n4 float4 groups (4 cells each), grid-stride.
+template <class OP>
+__global__ void __launch_bounds__(kBlock)
+map_vec4(const float4 *__restrict__ s, const float4 *__restrict__ nx,
+         const float4 *__restrict__ ny, const float4 *__restrict__ nz,
+         float4 *__restrict__ out, int64_t n4) {
+    const int64_t stride = (int64_t)gridDim.x * kBlock;
+    for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < n4; i += stride) {
+        const float4 v = ld_stream(s + i);
+        const float4 a = ld_stream(nx + i);
+        const float4 b = ld_stream(ny + i);
+        const float4 c = ld_stream(nz + i);
+        float4 r;
+        r.x = OP::apply(v.x, a.x, b.x, c.x);
+        r.y = OP::apply(v.y, a.y, b.y, c.y);
+        r.z = OP::apply(v.z, a.z, b.z, c.z);
+        r.w = OP::apply(v.w, a.w, b.w, c.w);
+        st_stream(out + i, r);
+    }
+}
+
+// Scalar: cells [0, head) and [tail0, N) (head/tail of the vector body), or the whole
+// range when the five pointers do not share an alignment (head = N).
+template <class OP>
+__global__ void __launch_bounds__(kBlock)
+map_scalar(const float *__restrict__ s, const float *__restrict__ nx,
+           const float *__restrict__ ny, const float *__restrict__ nz,
+           float *__restrict__ out, int64_t head, int64_t tail0, int64_t N) {
+    const int64_t stride = (int64_t)gridDim.x * kBlock;
+    const int64_t count = head + (N - tail0);
+    for (int64_t j = (int64_t)blockIdx.x * kBlock + threadIdx.x; j < count; j += stride) {
+        const int64_t i = j < head ? j : tail0 + (j - head);
+        out[i] = OP::apply(s[i], nx[i], ny[i], nz[i]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// launch geometry: persistent grid = SMs x resident blocks per SM, cached per device/kernel
+// ---------------------------------------------------------------------------------------
+constexpr int kNumKernels = 2 * PLIC_NUM_METHODS + 1;      // 8 solve variants + volume
+
+struct DeviceInfo {
+    std::once_flag once;
+    int sms = 0;
+    int blocks_per_sm[kNumKernels] = {0};
+    cudaError_t err = cudaSuccess;
+};
+static DeviceInfo g_dev[kMaxDevices];
+static std::atomic<int64_t> g_launches{0};
+
+typedef void (*vec_kernel_t)(const float4 *, const float4 *, const float4 *, const float4 *,
+                             float4 *, int64_t);
+typedef void (*scalar_kernel_t)(const float *, const float *, const float *, const float *,
+                                float *, int64_t, int64_t, int64_t);
+
+static vec_kernel_t vec_kernel(int k) {
+    switch (k) {
+        case 0: return map_vec4<SolveOp<ANALYTIC, false>>;
+        case 1: return map_vec4<SolveOp<SZ, false>>;
+        case 2: return map_vec4<SolveOp<NEWTON, false>>;
+        case 3: return map_vec4<SolveOp<NESTED, false>>;
+        case 4: return map_vec4<SolveOp<ANALYTIC, true>>;
+        case 5: return map_vec4<SolveOp<SZ, true>>;
+        case 6: return map_vec4<SolveOp<NEWTON, true>>;
+        case 7: return map_vec4<SolveOp<NESTED, true>>;
+        default: return map_vec4<VolumeOp>;
+    }
+}
+static scalar_kernel_t scalar_kernel(int k) {
+    switch (k) {
+        case 0: return map_scalar<SolveOp<ANALYTIC, false>>;
+        case 1: return map_scalar<SolveOp<SZ, false>>;
+        case 2: return map_scalar<SolveOp<NEWTON, false>>;
+        case 3: return map_scalar<SolveOp<NESTED, false>>;
+        case 4: return map_scalar<SolveOp<ANALYTIC, true>>;
+        case 5: return map_scalar<SolveOp<SZ, true>>;
+        case 6: return map_scalar<SolveOp<NEWTON, true>>;
+        case 7: return map_scalar<SolveOp<NESTED, true>>;
+        default: return map_scalar<VolumeOp>;
+    }
+}
+
+// kernel index for a method id; -1 if the id is unknown
+static int kernel_index(int method) {
+    const int base = method & ~PLIC_FAST;
+    if (base < 0 || base >= PLIC_NUM_METHODS) return -1;
+    return base + ((method & PLIC_FAST) ? PLIC_NUM_METHODS : 0);
+}
+constexpr int kVolumeKernel = 2 * PLIC_NUM_METHODS;
+
+static DeviceInfo *device_info(cudaError_t *err) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess || dev < 0 || dev >= kMaxDevices) {
+        *err = e != cudaSuccess ? e : cudaErrorInvalidDevice;
+        return nullptr;
+    }
+    DeviceInfo *info = &g_dev[dev];
+    std::call_once(info->once, [info, dev]() {
+        cudaError_t e2 = cudaDeviceGetAttribute(&info->sms, cudaDevAttrMultiProcessorCount, dev);
+        for (int k = 0; k < kNumKernels && e2 == cudaSuccess; ++k) {
+            e2 = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&info->blocks_per_sm[k],
+                                                               vec_kernel(k), kBlock, 0);
+            if (info->blocks_per_sm[k] < 1) info->blocks_per_sm[k] = 1;
+        }
+        info->err = e2;
+    });
+    *err = info->err;
+    return info->err == cudaSuccess ? info : nullptr;
+}
+
+static int grid_for(const DeviceInfo *info, int k, int64_t n4) {
+    const int64_t full = (int64_t)info->sms * info->blocks_per_sm[k];
+    const int64_t need = (n4 + kBlock - 1) / kBlock;
+    return (int)(need < full ? (need < 1 ? 1 : need) : full);
+}
+
+static int launch_map(int k, const float *s, const float *nx, const float *ny, const float *nz,
+                      float *out, int64_t N, cudaStream_t stream) {
+    if (N < 0) return PLIC_ERR_SIZE;
+    if (N == 0) return PLIC_OK;
+    if (!s || !nx || !ny || !nz || !out) return PLIC_ERR_NULL;
+    const uintptr_t ps[5] = {(uintptr_t)s, (uintptr_t)nx, (uintptr_t)ny, (uintptr_t)nz,
+                             (uintptr_t)out};
+    bool same = true;
+    for (int i = 0; i < 5; ++i) {
+        if (ps[i] & 3u) return PLIC_ERR_ALIGN;
+        if ((ps[i] & 15u) != (ps[0] & 15u)) same = false;
+    }
+    cudaError_t err;
+    const DeviceInfo *info = device_info(&err);
+    if (!info) return PLIC_ERR_LAUNCH;
+
+    // cells before the first 16-byte boundary, then n4 full float4 groups, then the tail
+    int64_t head = same ? (int64_t)(((16u - (ps[0] & 15u)) & 15u) >> 2) : N;
+    if (head > N) head = N;
+    const int64_t n4 = (N - head) / 4;
+    const int64_t tail0 = head + 4 * n4;
+
+    if (n4 > 0) {
+        vec_kernel(k)<<<grid_for(info, k, n4), kBlock, 0, stream>>>(
+            (const float4 *)(s + head), (const float4 *)(nx + head), (const float4 *)(ny + head),
+            (const float4 *)(nz + head), (float4 *)(out + head), n4);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+    }
+    const int64_t rest = head + (N - tail0);
+    if (rest > 0) {
+        scalar_kernel(k)<<<grid_for(info, k, rest), kBlock, 0, stream>>>(s, nx, ny, nz, out, head,
+                                                                      tail0, N);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+    }
+    return cudaGetLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
+}
+
+// ---------------------------------------------------------------------------------------
+// host-array API: chunked, three-stage pipeline (H2D | kernel | D2H) over three streams
+// ---------------------------------------------------------------------------------------
+constexpr int kSlots = 3;
+constexpr int64_t kChunk = (int64_t)1 << 22;     // cells per chunk: 64 MiB in, 16 MiB out
+
+struct HostPipe {
+    bool ready = false;
+    cudaStream_t stream[kSlots] = {nullptr, nullptr, nullptr};
+    float *buf[kSlots] = {nullptr, nullptr, nullptr};     // 5 * kChunk floats each
+};
+static HostPipe g_pipe[kMaxDevices];
+static std::mutex g_pipe_mutex;
+
+static void pipe_free(HostPipe *p) {
+    for (int i = 0; i < kSlots; ++i) {
+        if (p->buf[i]) cudaFree(p->buf[i]);
+        if (p->stream[i]) cudaStreamDestroy(p->stream[i]);
+        p->buf[i] = nullptr;
+        p->stream[i] = nullptr;
+    }
+    p->ready = false;
+}
+
+static bool pipe_init(HostPipe *p) {
+    if (p->ready) return true;
+    for (int i = 0; i < kSlots; ++i) {
+        if (cudaStreamCreateWithFlags(&p->stream[i], cudaStreamNonBlocking) != cudaSuccess ||
+            cudaMalloc((void **)&p->buf[i], 5 * kChunk * sizeof(float)) != cudaSuccess) {
+            pipe_free(p);
+            cudaGetLastError();
+            return false;
+        }
+    }
+    p->ready = true;
+    return true;
+}
+
+static int host_map(int k, const float *s, const float *nx, const float *ny, const float *nz,
+                    float *out, int64_t N) {
+    if (N < 0) return PLIC_ERR_SIZE;
+    if (N == 0) return PLIC_OK;
+    if (!s || !nx || !ny || !nz || !out) return PLIC_ERR_NULL;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return PLIC_ERR_LAUNCH;
+    std::lock_guard<std::mutex> lock(g_pipe_mutex);
+    HostPipe *p = &g_pipe[dev];
+    if (!pipe_init(p)) return PLIC_ERR_LAUNCH;
+    const float *in[4] = {s, nx, ny, nz};
+    int rc = PLIC_OK;
+    int slot = 0;
+    for (int64_t off = 0; off < N && rc == PLIC_OK; off += kChunk, slot = (slot + 1) % kSlots) {
+        const int64_t n = (N - off) < kChunk ? (N - off) : kChunk;
+        cudaStream_t st = p->stream[slot];     // stream order makes the slot's reuse safe
+        float *b = p->buf[slot];
+        for (int a = 0; a < 4; ++a)
+            if (cudaMemcpyAsync(b + a * kChunk, in[a] + off, n * sizeof(float),
+                                cudaMemcpyHostToDevice, st) != cudaSuccess)
+                rc = PLIC_ERR_LAUNCH;
+        if (rc == PLIC_OK)
+            rc = launch_map(k, b, b + kChunk, b + 2 * kChunk, b + 3 * kChunk, b + 4 * kChunk, n, st);
+        if (rc == PLIC_OK &&
+            cudaMemcpyAsync(out + off, b + 4 * kChunk, n * sizeof(float), cudaMemcpyDeviceToHost,
+                            st) != cudaSuccess)
+            rc = PLIC_ERR_LAUNCH;
+    }
+    for (int i = 0; i < kSlots; ++i)
+        if (cudaStreamSynchronize(p->stream[i]) != cudaSuccess) rc = PLIC_ERR_LAUNCH;
+    if (rc != PLIC_OK) cudaGetLastError();
+    return rc;
+}
+
+}  // namespace plic
+
+// ---------------------------------------------------------------------------------------
+// C ABI
+// ---------------------------------------------------------------------------------------
+extern "C" {
+
+int plic_solve(const float *V0, const float *nx, const float *ny, const float *nz, float *d0,
+               int64_t N, int method, cudaStream_t stream) {
+    const int k = plic::kernel_index(method);
+    if (k < 0) return PLIC_ERR_METHOD;
+    return plic::launch_map(k, V0, nx, ny, nz, d0, N, stream);
+}
+
+int plic_volume(const float *d0, const float *nx, const float *ny, const float *nz, float *V0,
+                int64_t N, cudaStream_t stream) {
+    return plic::launch_map(plic::kVolumeKernel, d0, nx, ny, nz, V0, N, stream);
+}
+
+int plic_solve_host(const float *V0, const float *nx, const float *ny, const float *nz,
+                    float *d0, int64_t N, int method) {
+    const int k = plic::kernel_index(method);
+    if (k < 0) return PLIC_ERR_METHOD;
+    return plic::host_map(k, V0, nx, ny, nz, d0, N);
+}
+
+int plic_volume_host(const float *d0, const float *nx, const float *ny, const float *nz,
+                     float *V0, int64_t N) {
+    return plic::host_map(plic::kVolumeKernel, d0, nx, ny, nz, V0, N);
+}
+
+void plic_host_release(void) {
+    std::lock_guard<std::mutex> lock(plic::g_pipe_mutex);
+    int cur = 0;
+    const bool have = cudaGetDevice(&cur) == cudaSuccess;
+    for (int d = 0; d < plic::kMaxDevices; ++d) {
+        if (!plic::g_pipe[d].ready) continue;
+        cudaSetDevice(d);
+        plic::pipe_free(&plic::g_pipe[d]);
+    }
+    if (have) cudaSetDevice(cur);
+}
+
+const char *plic_method_name(int method) {
+    static const char *names[2 * PLIC_NUM_METHODS] = {
+        "analytic",      "sz",      "newton",      "nested",
+        "analytic-fast", "sz-fast", "newton-fast", "nested-fast"};
+    const int k = plic::kernel_index(method);
+    return k < 0 ? nullptr : names[k];
+}
+
+const char *plic_error_string(int code) {
+    switch (code) {
+        case PLIC_OK: return "ok";
+        case PLIC_ERR_NULL: return "null pointer with N > 0";
+        case PLIC_ERR_SIZE: return "negative N";
+        case PLIC_ERR_METHOD: return "unknown method id";
+        case PLIC_ERR_LAUNCH: return "CUDA runtime error";
+        case PLIC_ERR_ALIGN: return "pointer not 4-byte aligned";
+        default: return "unknown error code";
+    }
+}
+
+int plic_version(void) { return PLIC_VERSION; }
+
+int plic_launch_config(int method, int64_t N, int *grid, int *block, int *cells_per_thread) {
+    const int k = method == -1 ? plic::kVolumeKernel : plic::kernel_index(method);
+    if (k < 0) return PLIC_ERR_METHOD;
+    if (N < 0) return PLIC_ERR_SIZE;
+    if (!grid || !block || !cells_per_thread) return PLIC_ERR_NULL;
+    cudaError_t err;
+    const plic::DeviceInfo *info = plic::device_info(&err);
+    if (!info) return PLIC_ERR_LAUNCH;
+    *grid = plic::grid_for(info, k, N / 4);
+    *block = plic::kBlock;
+    *cells_per_thread = 4;
+    return PLIC_OK;
+}
+
+int64_t plic_launch_count(void) { return plic::g_launches.load(std::memory_order_relaxed); }
+
+}  // extern "C"

@@ -1,0 +1,390 @@
+// plic_methods.cuh -- per-cell fp32 device functions of the PLIC hot path (sm_100a).
+//
+// PAPER.md = /root/reference/PAPER.md (arxiv 2006.12838).  Notation follows the paper:
+//   n1 <= n2 <= n3   mirrored, sorted normal components        eq. (2)-(4)
+//   V in [0, 1/2]    reduced volume                            eq. (5),
+//   d in [0, S/2]    reduced offset from the cube corner       eq. (7),
+//   (1)..(5)         the five intersection cases               eq. (11),
+// and, as shorthands used throughout:
+//   n12 = n1+n2, S = n1+n2+n3, q = n1 n2, W = 2 V n3, z = n12 - W, e = n3 - n12,
+//   x = 6 V n2 n3 = 3 W n2,  u = 4 q - e^2  ( = S^2 - 2 sum n_i^2; = t4/9 of eq. (19) when |n|=1 ).
+//
+// Each method is `reduced_offset<METHOD, FAST>(n1, n2, n3, V) -> d`; the frame solve_cell()
+// does the symmetry reduction before and the sign restore (eq. (8)) after.  The bodies of
+// the paper's Listings 1, 2, 4, 5, 6 are not in PAPER.md (captions only) and Listing 3 is
+// truncated, so every method is built from the equations; DESIGN.md lists the readings.
+//
+// Cases (3) and (4) are cubics in d.  All methods use them in depressed form
+//   F(tau) = tau^3 - p tau - r = 0,  d = base + tau:
+//   case (3): base = n12, p = 6 q,     r = 3 q z,          tau in [-n1, min(0, e)]
+//   case (4): base = S/2, p = 3 u / 4, r = 3 q (n3 - W)/2, tau in [n3 - S/2, 0]
+// (expand eq. (11) around d = n12 resp. d = S/2), because every coefficient is then a
+// product of small quantities and no cancellation of O(1) terms occurs when n1 is small.
+// The trigonometric root of these cubics is
+//   tau = -2 sqrt(p/3) sin(asin(C)/3),  C = (r/2) (3/p)^(3/2),
+// which is eq. (12) with atan2(y,x) = acos(C) and pi/6 - acos(C)/3 = asin(C)/3:
+//   case (3): d = n12 - 2 sqrt(2 q) sin(asin(C3)/3), C3 = 3 z / (4 sqrt(2 q))
+//   case (4): d = S/2 - sqrt(u)     sin(asin(C4)/3), C4 = 6 q (n3 - W) / u^(3/2).
+// Which of (3)/(4) applies is decided a priori by the sign of F3(e) (d3 <= n3  <=>  F3(e) <= 0,
+// F3 being decreasing on [-n1, 0]), or a posteriori by d3 <= n3 as the paper does
+// (PAPER.md:151), where noted.
+#pragma once
+#include "plic_math.cuh"
+
+namespace plic {
+
+enum : int { ANALYTIC = 0, SZ = 1, NEWTON = 2, NESTED = 3 };
+
+// ---------------------------------------------------------------------------------------
+// shared pieces
+// ---------------------------------------------------------------------------------------
+
+// A-priori (3)-vs-(4) decision: case (4) iff n3 < n12 and F3(e) > 0.
+__device__ __forceinline__ bool is_case4(float q, float e, float ee, float z) {
+    const float h = fmaf(fmaf(-6.0f, q, ee), e, -3.0f * (q * z));
+    return (e < 0.0f) && (h > 0.0f);
+}
+
+// Newton-Raphson on F(tau) = tau^3 - p tau - r:  tau <- (2 tau^3 + r) / (3 tau^2 - p).
+template <bool FAST, int ITERS>
+__device__ __forceinline__ float newton_cubic(float p, float r, float tau) {
+#pragma unroll
+    for (int i = 0; i < ITERS; ++i) {
+        const float t2 = tau * tau;
+        tau = Math<FAST>::div(fmaf(2.0f * t2, tau, r), fmaf(3.0f, t2, -p));
+    }
+    return tau;
+}
+
+// Start value for the cube root of k > 0: exponent/3 by integer arithmetic (relative error
+// <= 3.2 %; the constant minimises the maximum error over [1e-30, 1]).
+__device__ __forceinline__ float cbrt_seed(float k) {
+    return __int_as_float(__float_as_int(k) / 3 + 0x2a510680);
+}
+
+// ---------------------------------------------------------------------------------------
+// method 0: the paper's analytic inverse, eq. (25)/(26), order (5)->(2)->(1)->(3)->(4)
+// ---------------------------------------------------------------------------------------
+template <int METHOD, bool FAST>
+struct Solver;
+
+// Precise: branches in the paper's order, a-posteriori d3 <= n3.
+template <>
+struct Solver<ANALYTIC, false> {
+    static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
+        typedef Math<false> M;
+        const float n12 = n1 + n2;
+        const float W = 2.0f * V * n3;
+        if (n12 <= W) return fmaf(V, n3, 0.5f * n12);                      // (5) eq. (26)
+        const float x = 3.0f * W * n2;
+        const float s1 = n1 * n1;
+        if (x >= s1) {
+            // (2): n1^2 <= 6 V n2 n3 <= n1^2 + 3 n2 (n2 - n1)   [eq. (26), misprint corrected]
+            if (x <= fmaf(3.0f * n2, n2 - n1, s1))
+                return fmaf(0.5f, n1, M::sqrt(fmaxf(fmaf(W, n2, -s1 * (1.0f / 12.0f)), 0.0f)));
+        } else {
+            return M::cbrt(x * n1);                                        // (1)
+        }
+        const float q = n1 * n2;
+        const float sq = M::sqrt(q + q);
+        const float C3 = 0.75f * M::div(n12 - W, sq);
+        const float d3 = fmaf(-2.0f * sq, M::sin_third_asin(C3), n12);     // (3)
+        if (d3 <= n3) return fmaxf(d3, n2);
+        const float e = n3 - n12;
+        const float u = fmaf(4.0f, q, -e * e);
+        const float su = M::sqrt(u);
+        const float C4 = M::div(6.0f * q * (n3 - W), u * su);
+        const float d4 = fmaf(-su, M::sin_third_asin(C4), 0.5f * (n12 + n3));   // (4)
+        return fmaxf(d4, n3);
+    }
+};
+
+// One trigonometric evaluation serving (3) and (4): parameters selected, then evaluated once.
+template <bool FAST>
+__device__ __forceinline__ float trig_case34(float n1, float n2, float n3, float n12, float W) {
+    const float q = n1 * n2;
+    const float e = n3 - n12;
+    const float z = n12 - W;
+    const float ee = e * e;
+    const bool c4 = is_case4(q, e, ee, z);
+    const float u = fmaf(4.0f, q, -ee);
+    const float X = c4 ? u : q + q;
+    const float r = mufu_rsqrt(X);
+    const float Xr = X * r;                                   // sqrt(X)
+    const float K = c4 ? 6.0f * q * (n3 - W) * (r * r) : 0.75f * z;
+    const float g = Math<FAST>::sin_third_asin(K * r);
+    const float B = c4 ? Xr : Xr + Xr;
+    const float A = c4 ? 0.5f * (n12 + n3) : n12;
+    return fmaxf(fmaf(-B, g, A), c4 ? n3 : n2);               // bracket floor; also drops NaN
+}
+
+// Fast: every closed form evaluated, merged by select; (3)/(4) share one trig evaluation.
+template <>
+struct Solver<ANALYTIC, true> {
+    static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
+        typedef Math<true> M;
+        const float n12 = n1 + n2;
+        const float W = (V + V) * n3;
+        const float x = 3.0f * W * n2;
+        const float s1 = n1 * n1;
+        const bool c5 = n12 <= W;
+        const float d2 = fmaf(0.5f, n1, M::sqrt(fmaxf(fmaf(W, n2, -s1 * (1.0f / 12.0f)), 0.0f)));
+        const float d1 = M::cbrt(x * n1);
+        float d = x < s1 ? d1 : d2;
+        if (!c5 && x > fmaf(3.0f * n2, n2 - n1, s1)) d = trig_case34<true>(n1, n2, n3, n12, W);
+        return c5 ? 0.5f * (W + n12) : d;
+    }
+};
+
+// ---------------------------------------------------------------------------------------
+// method 1: Scardovelli-Zaleski, edge-case complete and micro-optimised (sect. 2.4)
+//
+// L1-normalised m_i = n_i / S, alpha = d / S, w = V.  Cases chosen a priori
+// from volume thresholds multiplied through so that nothing divides by m1 or m2, with (5)
+// and (2) tested first.  The cubic of Listing 3,
+//   case (3): a2 = -3 m12, a1 = 3 (m1^2+m2^2),    a0 = w6 - m1^3 - m2^3
+//   case (4): a2 = -3/2,   a1 = 3/2 sum m_i^2,    a0 = (w6 - sum m_i^3)/2,   w6 = 6 m1 m2 m3 w
+// is solved by the trigonometric root
+//   p0 = a2^2/9 - a1/3, q0 = (a1 a2 - 3 a0)/6 - a2^3/27,
+//   alpha = 2 sqrt(p0) cos( acos(q0 / p0^(3/2)) / 3 + 4 pi / 3 ) - a2/3
+// with p0 and q0 collapsed algebraically (using m1+m2+m3 = 1) to
+//   case (3): p0 = 2 m1 m2,                   q0 = 3/2 m1 m2 (m12 - 2 w m3)
+//   case (4): p0 = m1 m2 - (m12 - m3)^2 / 4,  q0 = 3/4 m1 m2 m3 (1 - 2 w)
+// -- the literal a2, a1, a0 arithmetic loses all significance in fp32 when m1 is small
+// ("SZ cancellation").
+// ---------------------------------------------------------------------------------------
+template <bool FAST>
+struct Solver<SZ, FAST> {
+    static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
+        typedef Math<FAST> M;
+        const float S = (n1 + n2) + n3;
+        const float inv = M::div(1.0f, S);
+        const float m1 = n1 * inv, m2 = n2 * inv, m3 = n3 * inv;
+        const float m12 = m1 + m2;
+        const float w = V;
+        const float W = 2.0f * w * m3;
+        float alpha;
+        if (m12 <= W) {
+            alpha = fmaf(w, m3, 0.5f * m12);                                   // (5)
+        } else {
+            const float x = 3.0f * W * m2;                                     // 6 w m2 m3
+            const float s1 = m1 * m1;                                          // w < v1 <=> x < m1^2
+            if (x >= s1 && x <= fmaf(3.0f * m2, m2 - m1, s1)) {                // (2): v1 <= w <= v2
+                alpha = 0.5f * (m1 + M::sqrt(fmaxf(fmaf(4.0f * W, m2, -s1 * (1.0f / 3.0f)), 0.0f)));
+            } else if (x < s1) {
+                alpha = M::cbrt(x * m1);                                       // (1): cbrt(w6)
+            } else {
+                const float q = m1 * m2;
+                bool c4 = false;
+                if (m3 < m12) {
+                    // 6 m1 m2 m3 v3 of Listing 3; case (4) iff w6 >= it
+                    const float s2 = m2 * m2;
+                    float v3n = m3 * m3 * fmaf(3.0f, m12, -m3);
+                    v3n = fmaf(s1, fmaf(-3.0f, m3, m1), v3n);
+                    v3n = fmaf(s2, fmaf(-3.0f, m3, m2), v3n);
+                    c4 = x * m1 >= v3n;
+                }
+                const float em = m12 - m3;
+                const float p0 = c4 ? fmaf(-0.25f * em, em, q) : q + q;
+                const float q0 = c4 ? 0.75f * q * (m3 - W) : 1.5f * q * (m12 - W);
+                const float sp = M::sqrt(p0);
+                const float theta = M::acos(M::div(q0, p0 * sp)) * (1.0f / 3.0f);
+                // cos(theta + 4 pi/3) evaluated as cos(theta - 2 pi/3): same angle, |arg| < pi
+                alpha = fmaf(2.0f * sp, M::cos(theta - 2.0943951f), c4 ? 0.5f : m12);
+                alpha = fmaxf(alpha, c4 ? m3 : m2);                            // bracket floor
+            }
+        }
+        return alpha * S;
+    }
+};
+
+// ---------------------------------------------------------------------------------------
+// method 2: Newton-Raphson for cases (1), (3), (4); closed forms for (2), (5)  (sect. 2.5)
+// Fixed, unrolled trip counts: case (1) on d^3 - 6 V n1 n2 n3 from the
+// integer-arithmetic seed, cases (3)/(4) on the depressed cubics from the top of the bracket
+// (tau0 = min(0, e) resp. 0), where F is decreasing and concave so the iteration is monotone.
+// ---------------------------------------------------------------------------------------
+template <>
+struct Solver<NEWTON, false> {
+    static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
+        typedef Math<false> M;
+        const float n12 = n1 + n2;
+        const float W = 2.0f * V * n3;
+        if (n12 <= W) return fmaf(V, n3, 0.5f * n12);                      // (5)
+        const float x = 3.0f * W * n2;
+        const float s1 = n1 * n1;
+        if (x >= s1) {
+            if (x <= fmaf(3.0f * n2, n2 - n1, s1))                         // (2)
+                return fmaf(0.5f, n1, M::sqrt(fmaxf(fmaf(W, n2, -s1 * (1.0f / 12.0f)), 0.0f)));
+        } else {
+            const float k = x * n1;                                        // (1)
+            return newton_cubic<false, 3>(0.0f, k, cbrt_seed(k));
+        }
+        const float q = n1 * n2;
+        const float e = n3 - n12;
+        const float z = n12 - W;
+        const float ee = e * e;
+        if (is_case4(q, e, ee, z)) {                                       // (4)
+            const float u = fmaf(4.0f, q, -ee);
+            const float s = newton_cubic<false, 4>(0.75f * u, 1.5f * q * (n3 - W), 0.0f);
+            return fmaxf(0.5f * (n12 + n3) + s, n3);
+        }
+        const float t = newton_cubic<false, 4>(6.0f * q, 3.0f * q * z, fminf(e, 0.0f));   // (3)
+        return fmaxf(n12 + t, n2);
+    }
+};
+
+// Fast: one unrolled Newton loop serves (1), (3) and (4) with per-case (p, r, tau0, base).
+template <>
+struct Solver<NEWTON, true> {
+    static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
+        typedef Math<true> M;
+        const float n12 = n1 + n2;
+        const float W = (V + V) * n3;
+        const float x = 3.0f * W * n2;
+        const float s1 = n1 * n1;
+        const bool c5 = n12 <= W;
+        const bool c1 = x < s1;
+        float d = fmaf(0.5f, n1, M::sqrt(fmaxf(fmaf(W, n2, -s1 * (1.0f / 12.0f)), 0.0f)));   // (2)
+        if (!c5 && (c1 || x > fmaf(3.0f * n2, n2 - n1, s1))) {
+            const float q = n1 * n2;
+            const float e = n3 - n12;
+            const float z = n12 - W;
+            const float ee = e * e;
+            const bool c4 = is_case4(q, e, ee, z);
+            const float k = x * n1;
+            float p = c4 ? 0.75f * fmaf(4.0f, q, -ee) : 6.0f * q;
+            float r = c4 ? 1.5f * q * (n3 - W) : 3.0f * q * z;
+            float tau = c4 ? 0.0f : fminf(e, 0.0f);
+            float base = c4 ? 0.5f * (n12 + n3) : n12;
+            float floor_ = c4 ? n3 : n2;
+            if (c1) { p = 0.0f; r = k; tau = cbrt_seed(k); base = 0.0f; floor_ = 0.0f; }
+            d = fmaxf(base + newton_cubic<true, 4>(p, r, tau), floor_);
+        }
+        return c5 ? 0.5f * (W + n12) : d;
+    }
+};
+
+// ---------------------------------------------------------------------------------------
+// method 3: nested intervals (bisection) for cases (3), (4); closed forms otherwise (sect. 2.5)
+// F is decreasing on the bracket [lo, hi] with F(lo) >= 0 >= F(hi).
+// ---------------------------------------------------------------------------------------
+// Precise: halve until the fp32 midpoint stops moving -- a data-dependent trip count that
+// grows with the initial width, as the paper describes ("not unrolled").
+__device__ __forceinline__ float bisect_cubic_converged(float p, float r, float lo, float hi) {
+    for (int i = 0; i < 64; ++i) {
+        const float mid = 0.5f * (lo + hi);
+        if (!(mid > lo && mid < hi)) break;
+        const float F = fmaf(fmaf(mid, mid, -p), mid, -r);
+        if (F > 0.0f) lo = mid; else hi = mid;
+    }
+    return 0.5f * (lo + hi);
+}
+
+// Fast: a fixed number of halvings, branch-free (lo, width) form.
+template <int HALVINGS>
+__device__ __forceinline__ float bisect_cubic_fixed(float p, float r, float lo, float hi) {
+    float w = hi - lo;
+#pragma unroll
+    for (int i = 0; i < HALVINGS; ++i) {
+        w *= 0.5f;
+        const float mid = lo + w;
+        const float F = fmaf(fmaf(mid, mid, -p), mid, -r);
+        lo = F > 0.0f ? mid : lo;
+    }
+    return fmaf(0.5f, w, lo);
+}
+
+template <bool FAST>
+struct Solver<NESTED, FAST> {
+    static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
+        typedef Math<FAST> M;
+        const float n12 = n1 + n2;
+        const float W = 2.0f * V * n3;
+        const bool c5 = n12 <= W;
+        const float x = 3.0f * W * n2;
+        const float s1 = n1 * n1;
+        float d;
+        if (x < s1) {
+            d = M::cbrt(x * n1);                                               // (1)
+        } else {
+            d = fmaf(0.5f, n1, M::sqrt(fmaxf(fmaf(W, n2, -s1 * (1.0f / 12.0f)), 0.0f)));   // (2)
+        }
+        if (!c5 && x > fmaf(3.0f * n2, n2 - n1, s1)) {
+            const float q = n1 * n2;
+            const float e = n3 - n12;
+            const float z = n12 - W;
+            const float ee = e * e;
+            const bool c4 = is_case4(q, e, ee, z);
+            const float hS = 0.5f * (n12 + n3);
+            const float p = c4 ? 0.75f * fmaf(4.0f, q, -ee) : 6.0f * q;
+            const float r = c4 ? 1.5f * q * (n3 - W) : 3.0f * q * z;
+            const float lo = c4 ? n3 - hS : -n1;
+            const float hi = c4 ? 0.0f : fminf(e, 0.0f);
+            const float tau = FAST ? bisect_cubic_fixed<20>(p, r, lo, hi)
+                                   : bisect_cubic_converged(p, r, lo, hi);
+            d = (c4 ? hS : n12) + tau;
+        }
+        return c5 ? fmaf(V, n3, 0.5f * n12) : d;
+    }
+};
+
+// ---------------------------------------------------------------------------------------
+// frame: symmetry reduction (eq. (2)-(5)) -> method -> sign restore (eq. (8))
+// ---------------------------------------------------------------------------------------
+template <int METHOD, bool FAST>
+__device__ __forceinline__ float solve_cell(float V0, float nx, float ny, float nz) {
+    const float a = fabsf(nx), b = fabsf(ny), c = fabsf(nz);
+    const float n1 = min3(a, b, c);                                    // eq. (2)
+    const float n3 = max3(a, b, c);                                    // eq. (3)
+    const float n2 = fmaxf(fminf(a, b), fminf(fmaxf(a, b), c));        // eq. (4): the median
+    // eq. (5): 1/2 - |V0 - 1/2| = min(V0, 1 - V0), which is exact in fp32 for V0 in [0,1]
+    const float V = fmaxf(fminf(V0, 1.0f - V0), 0.0f);
+    float d = Solver<METHOD, FAST>::reduced_offset(n1, n2, n3, V);
+    const float hS = 0.5f * ((n1 + n2) + n3);
+    d = fminf(fmaxf(d, 0.0f), hS);                                     // d in [0, S/2]; drops NaN
+    const float r = hS - d;
+    return V0 > 0.5f ? r : -r;                                         // eq. (8)
+}
+
+// ---------------------------------------------------------------------------------------
+// forward map V0(d0, n): eq. (2)-(4), (7), (11), (6)   (Listing 1)
+//
+// Case (5) first and case (2) in its n1-free form, so n1 = 0 and n1 = n2 = 0 never divide
+// by zero (caption of Listing 1).  Cases (3) and (4) are evaluated in the expanded forms
+//   (3): V = (n12/2 + t - t^3/(6 n1 n2)) / n3,                 t = d - n12 in [-n1, 0]
+//   (4): V = 1/2 + s (3 u/4 - s^2) / (3 n1 n2 n3),             s = d - S/2 in [-n1/2, 0]
+// instead of the fdim-merged difference of cubes of Listing 1: that difference cancels to
+// ~eps d^3/(6 n1 n2 n3) in fp32, i.e. 4e-3 for n1 = 1e-6 ("forward map").
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ float volume_cell(float d0, float nx, float ny, float nz) {
+    const float a = fabsf(nx), b = fabsf(ny), c = fabsf(nz);
+    const float n1 = min3(a, b, c);
+    const float n3 = max3(a, b, c);
+    const float n2 = fmaxf(fminf(a, b), fminf(fmaxf(a, b), c));
+    const float n12 = n1 + n2;
+    const float hS = 0.5f * (n12 + n3);
+    const float d = fmaxf(hS - fabsf(d0), 0.0f);                        // eq. (7)
+    float V;
+    if (n3 == 0.0f) {
+        V = d0 == 0.0f ? 0.5f : 0.0f;                                   // zero normal
+    } else if (d >= n12) {
+        V = (d - 0.5f * n12) / n3;                                      // (5)
+    } else if (d < n1) {
+        V = (d * d) / (6.0f * n2 * n3) * (d / n1);                      // (1)
+    } else if (d <= n2) {
+        V = fmaf(3.0f * d, d - n1, n1 * n1) / (6.0f * n2 * n3);         // (2)
+    } else if (d <= n3) {
+        const float t = d - n12;                                        // (3)
+        V = (fmaf(0.5f, n12, t) - (t * t) / (6.0f * n2) * (t / n1)) / n3;
+    } else {
+        const float e = n3 - n12;                                       // (4)
+        const float u = fmaf(4.0f, n1 * n2, -e * e);
+        const float s = d - hS;
+        V = fmaf(fmaf(0.75f, u, -s * s) / (3.0f * n2 * n3), s / n1, 0.5f);
+    }
+    V = fminf(fmaxf(V, 0.0f), 0.5f);
+    return d0 > 0.0f ? 1.0f - V : V;                                    // eq. (6)
+}
+
+}  // namespace plic

@@ -1,0 +1,113 @@
+"""CPU-side checks of the C-ABI boundary: libplic.so builds, loads, and exports every
+function include/plic.h declares; argument validation that returns before any CUDA call;
+method-id marshalling of the Python binding.  No compute happens here (there is no GPU and
+no CPU fallback)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def plic():
+    import paper_2006_12838_b200 as p
+    return p
+
+
+def _declared_functions():
+    src = open(os.path.join(ROOT, "include", "plic.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(plic_[a-z_]+)\s*\(", src)))
+
+
+def test_header_declares_the_boundary():
+    names = _declared_functions()
+    for must in ("plic_solve", "plic_volume", "plic_solve_host", "plic_volume_host",
+                 "plic_method_name", "plic_version", "plic_launch_count"):
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol(plic):
+    assert os.path.exists(plic.LIB_PATH)
+    raw = ctypes.CDLL(plic.LIB_PATH)
+    for name in _declared_functions():
+        assert hasattr(raw, name), name
+
+
+def test_header_compiles_as_plain_c(tmp_path):
+    import subprocess
+    c = tmp_path / "t.c"
+    c.write_text('#include "plic.h"\nint main(void){return PLIC_NUM_METHODS==4?0:1;}\n')
+    subprocess.run(["gcc", "-std=c11", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"),
+                    "-c", str(c), "-o", str(tmp_path / "t.o")], check=True)
+
+
+def test_version_and_names(plic):
+    assert plic.plic_version() == 100
+    assert [plic.plic_method_name(i) for i in range(4)] == ["analytic", "sz", "newton", "nested"]
+    assert plic.plic_method_name(2 | plic.FAST) == "newton-fast"
+    assert plic.plic_method_name(4) is None and plic.plic_method_name(-1) is None
+    assert plic.plic_error_string(0) == "ok"
+    for code in (-1, -2, -3, -4, -5):
+        assert plic.plic_error_string(code) not in ("ok", "unknown error code")
+
+
+def test_method_id_marshalling(plic):
+    assert plic.method_id("analytic") == 0
+    assert plic.method_id("sz", fast=True) == 0x101
+    assert plic.method_id("nested-fast") == 0x103
+    assert plic.method_id(2) == 2
+    with pytest.raises(ValueError):
+        plic.method_id("kawano")
+
+
+def test_argument_validation_needs_no_device(plic):
+    lib = plic.lib
+    buf = (ctypes.c_float * 8)()
+    p = ctypes.cast(buf, ctypes.c_void_p)
+    # N == 0: successful no-op, even with null pointers
+    assert lib.plic_solve(None, None, None, None, None, 0, 0, None) == 0
+    assert lib.plic_volume(None, None, None, None, None, 0, None) == 0
+    assert lib.plic_solve_host(None, None, None, None, None, 0, 0) == 0
+    # N < 0
+    assert lib.plic_solve(p, p, p, p, p, -1, 0, None) == -2
+    assert lib.plic_volume(p, p, p, p, p, -5, None) == -2
+    # null pointer with N > 0
+    assert lib.plic_solve(p, None, p, p, p, 4, 0, None) == -1
+    assert lib.plic_solve_host(p, p, p, p, None, 4, 0) == -1
+    # unknown method
+    assert lib.plic_solve(p, p, p, p, p, 4, 7, None) == -3
+    assert lib.plic_solve(p, p, p, p, p, 4, 0x204, None) == -3
+    assert lib.plic_solve_host(p, p, p, p, p, 4, -1) == -3
+    # misaligned (not a multiple of 4 bytes)
+    q = ctypes.c_void_p(p.value + 2)
+    assert lib.plic_solve(q, p, p, p, p, 1, 0, None) == -5
+    assert plic.plic_launch_count() == 0
+
+
+def test_binding_rejects_wrong_tensors(plic):
+    import numpy as np
+    import torch
+    a = torch.zeros(4)
+    with pytest.raises(ValueError):
+        plic.plic_solve(a, a, a, a)                       # CPU tensors on the device API
+    with pytest.raises(ValueError):
+        plic.plic_solve_host(np.zeros(4), np.zeros(4, np.float32), np.zeros(4, np.float32),
+                             np.zeros(4, np.float32))     # float64 array
+    with pytest.raises(ValueError):
+        plic.plic_solve_host(np.zeros(4, np.float32), np.zeros(3, np.float32),
+                             np.zeros(4, np.float32), np.zeros(4, np.float32))
+
+
+def test_no_oracle_in_product_path():
+    """The product (package, include/) never imports or links the oracle."""
+    pkg = os.path.join(ROOT, "paper_2006_12838_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt, f
+                assert "plic_oracle" not in txt, f

@@ -1,0 +1,346 @@
+"""GPU parity: the CUDA path (through the C ABI of libplic) against the fp64 CPU oracle,
+element by element on the same seeded inputs.
+
+Bars (BASELINE.json north_star): |d0 - d0_ref| <= 2e-5 absolute; forward-volume residual
+|V0_oracle(d0_gpu, n) - V0| <= 2e-5; finite everywhere, including n1 = 0, n1 = n2 = 0 and
+V0 in {0, 1/2, 1}.  plic_volume: |V0 - V0_ref| <= 1e-6 (DESIGN.md derives it from fp32
+rounding of the stable forms).  All eight plic_solve variants (4 methods x precise/fast).
+"""
+import os
+import sys
+
+import numpy as np
+import pytest
+import torch
+
+import gen
+import oracle
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+from stratified import stratified  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+TOL_D0 = 2e-5        # north_star
+TOL_RES = 2e-5       # north_star
+TOL_VOL = 1e-6
+
+VARIANTS = [(m, f) for m in ("analytic", "sz", "newton", "nested") for f in (False, True)]
+IDS = ["%s%s" % (m, "-fast" if f else "") for m, f in VARIANTS]
+
+
+@pytest.fixture(scope="module")
+def plic():
+    import paper_2006_12838_b200 as p
+    assert os.path.exists(p.LIB_PATH)
+    return p
+
+
+def dev(*arrays):
+    return [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in arrays]
+
+
+def check_solve(plic, V0, nx, ny, nz, method, fast, ref=None, what=""):
+    tV, tx, ty, tz = dev(V0, nx, ny, nz)
+    before = plic.plic_launch_count()
+    d0 = plic.plic_solve(tV, tx, ty, tz, method=method, fast=fast)
+    torch.cuda.synchronize()
+    assert plic.plic_launch_count() > before or len(V0) == 0     # the CUDA path ran
+    got = d0.cpu().numpy()
+    assert got.dtype == np.float32 and got.shape == V0.shape
+    assert np.all(np.isfinite(got)), "%s: non-finite d0" % what
+    if ref is None:
+        ref = oracle.solve(V0, nx, ny, nz)
+    err = np.abs(got.astype(np.float64) - ref)
+    i = int(np.argmax(err)) if len(err) else 0
+    assert err.max(initial=0.0) <= TOL_D0, "%s: |d0-ref| max %.3e at cell %d (V0=%r n=%r got=%r ref=%r)" % (
+        what, err.max(), i, V0[i], (nx[i], ny[i], nz[i]), got[i], ref[i])
+    res = np.abs(oracle.volume(got, nx, ny, nz) - np.clip(V0.astype(np.float64), 0.0, 1.0))
+    assert res.max(initial=0.0) <= TOL_RES, "%s: residual max %.3e" % (what, res.max())
+    S2 = 0.5 * (np.abs(nx.astype(np.float64)) + np.abs(ny) + np.abs(nz))
+    assert np.all(np.abs(got) <= S2 * (1 + 1e-6) + 1e-7)           # eq. (1): d0 in [-S/2, S/2]
+    return got, err
+
+
+# ------------------------------------------------------------------------------------------
+# config 1: 2^20 random + 4096 edge cells, seed 0, all variants
+# ------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def config1():
+    V0, nx, ny, nz = gen.config1(seed=0)
+    return V0, nx, ny, nz, oracle.solve(V0, nx, ny, nz)
+
+
+@pytest.mark.parametrize("method,fast", VARIANTS, ids=IDS)
+def test_config1_all_cells(plic, config1, method, fast):
+    V0, nx, ny, nz, ref = config1
+    assert V0.shape[0] == (1 << 20) + 4096
+    got, err = check_solve(plic, V0, nx, ny, nz, method, fast, ref, "config1")
+    edge = slice(1 << 20, None)
+    assert err[edge].max() <= TOL_D0
+    # exact volumes on the edge cells: V0 = 0 / 1 are the ends of the interval, 1/2 its centre
+    S2 = 0.5 * (np.abs(nx[edge]) + np.abs(ny[edge]) + np.abs(nz[edge])).astype(np.float64)
+    v = V0[edge]
+    assert np.max(np.abs(got[edge][v == 0.0] + S2[v == 0.0])) <= 2e-7
+    assert np.max(np.abs(got[edge][v == 1.0] - S2[v == 1.0])) <= 2e-7
+    assert np.max(np.abs(got[edge][v == 0.5])) <= 2e-7
+
+
+# ------------------------------------------------------------------------------------------
+# ragged sizes, misaligned pointers, aliasing, empty input
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("method,fast", VARIANTS, ids=IDS)
+def test_ragged_and_misaligned(plic, method, fast):
+    V0, nx, ny, nz = gen.random_sphere(70001, seed=11)
+    ref = oracle.solve(V0, nx, ny, nz)
+    tV, tx, ty, tz = dev(V0, nx, ny, nz)
+    for N in (0, 1, 2, 3, 4, 5, 7, 255, 256, 1023, 1027, 65537, 70001):
+        out = plic.plic_solve(tV[:N], tx[:N], ty[:N], tz[:N], method=method, fast=fast)
+        assert out.shape == (N,)
+        if N:
+            assert np.max(np.abs(out.cpu().numpy().astype(np.float64) - ref[:N])) <= TOL_D0
+    # common misalignment (head cells), offsets 1..3 floats
+    for off in (1, 2, 3):
+        N = 4099
+        out = torch.full((off + N + 5,), 7.0, device="cuda")
+        plic.plic_solve(tV[off:off + N], tx[off:off + N], ty[off:off + N], tz[off:off + N],
+                        out=out[off:off + N], method=method, fast=fast)
+        got = out.cpu().numpy()
+        assert np.all(got[:off] == 7.0) and np.all(got[off + N:] == 7.0)      # no overrun
+        assert np.max(np.abs(got[off:off + N].astype(np.float64) - ref[off:off + N])) <= TOL_D0
+    # mixed misalignment: scalar path for the whole range
+    N = 5001
+    out = plic.plic_solve(tV[1:1 + N], tx[2:2 + N].clone()[0:N], ty[3:3 + N], tz[0:N],
+                          method=method, fast=fast)
+    ref_mixed = oracle.solve(V0[1:1 + N], nx[2:2 + N], ny[3:3 + N], nz[0:N])
+    assert np.max(np.abs(out.cpu().numpy().astype(np.float64) - ref_mixed)) <= TOL_D0
+    # d0 may alias V0
+    a = tV.clone()
+    plic.plic_solve(a, tx, ty, tz, out=a, method=method, fast=fast)
+    assert np.max(np.abs(a.cpu().numpy().astype(np.float64) - ref)) <= TOL_D0
+
+
+def test_vector_and_scalar_paths_agree_bitwise(plic):
+    V0, nx, ny, nz = gen.random_sphere(50000, seed=12)
+    tV, tx, ty, tz = dev(V0, nx, ny, nz)
+    for method, fast in VARIANTS:
+        a = plic.plic_solve(tV, tx, ty, tz, method=method, fast=fast)
+        # force the scalar kernel: give one input a different alignment
+        sx = torch.empty(50001, device="cuda")[1:]
+        sx.copy_(tx)
+        b = plic.plic_solve(tV, sx, ty, tz, method=method, fast=fast)
+        assert torch.equal(a, b), (method, fast)
+
+
+# ------------------------------------------------------------------------------------------
+# the paper's own benchmark shape: axis normal, face diagonal, 12.5 % 2-D normals,
+# V0 equally spaced including 0 and 1; round-trip error of eq. (31)-(32)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("method,fast", VARIANTS, ids=IDS)
+def test_paper_benchmark_set_and_round_trip(plic, method, fast):
+    V0, nx, ny, nz = gen.paper_benchmark_set(2048, 257, seed=5)
+    got, _ = check_solve(plic, V0, nx, ny, nz, method, fast, None, "paper set")
+    # the Kawano NaN cells: n = (1,0,0), V0 in {0,1}
+    assert got[0] == -0.5 and got[256] == 0.5
+    tV, tx, ty, tz = dev(V0, nx, ny, nz)
+    back = plic.plic_volume(plic.plic_solve(tV, tx, ty, tz, method=method, fast=fast), tx, ty, tz)
+    E = (back - tV).abs()
+    # eq. (32): fp32 solvers reach E_avg of 2e-8 .. 7e-8 (Tables 1, 3); fast variants a bit above
+    assert float(E.mean()) < (3e-7 if fast else 1e-7), float(E.mean())
+    assert float(E.max()) < 2e-5
+
+
+# ------------------------------------------------------------------------------------------
+# config 3 shape: case-stratified, interleaved and case-contiguous
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("contiguous", [False, True], ids=["interleaved", "contiguous"])
+def test_case_stratified(plic, contiguous):
+    V0, nx, ny, nz, kase = stratified(1 << 19, seed=2, contiguous=contiguous)
+    ref = oracle.solve(V0, nx, ny, nz)
+    for method, fast in VARIANTS:
+        _, err = check_solve(plic, V0, nx, ny, nz, method, fast, ref, "stratified")
+        for k in range(1, 6):
+            assert (kase == k).sum() > 100000 and err[kase == k].max() <= TOL_D0
+
+
+# ------------------------------------------------------------------------------------------
+# config 4 shape: snapped normals (exact zeros, equal components), V0 ~ Beta(1/2,1/2)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("method,fast", VARIANTS, ids=IDS)
+def test_snapped_beta(plic, method, fast):
+    V0, nx, ny, nz = gen.snapped_beta(1 << 20, seed=3)
+    check_solve(plic, V0, nx, ny, nz, method, fast, None, "snapped")
+
+
+# ------------------------------------------------------------------------------------------
+# tiny smallest components: the regime where naive cubic arithmetic loses all digits
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("method,fast", VARIANTS, ids=IDS)
+def test_small_n1_sweep(plic, method, fast):
+    rng = np.random.default_rng(99)
+    m = 1 << 17
+    n1 = 10.0 ** rng.uniform(-12, -0.5, m)
+    ang = rng.uniform(0, 2 * np.pi, m)
+    g = np.stack([n1, np.cos(ang), np.sin(ang)], 1)
+    g /= np.linalg.norm(g, axis=1, keepdims=True)
+    perm = rng.permuted(np.tile(np.arange(3), (m, 1)), axis=1)
+    g = np.take_along_axis(g, perm, 1).astype(np.float32)
+    V0 = rng.random(m).astype(np.float32)
+    check_solve(plic, V0, g[:, 0].copy(), g[:, 1].copy(), g[:, 2].copy(), method, fast, None, "small n1")
+
+
+@pytest.mark.parametrize("method,fast", VARIANTS, ids=IDS)
+def test_degenerate_inputs(plic, method, fast):
+    s = np.float32(np.sqrt(0.5))
+    t = np.float32(1.0 / np.sqrt(3.0))
+    normals = [(1, 0, 0), (0, -1, 0), (0, 0, 1), (s, s, 0), (0, -s, s), (s, 0, -s), (t, t, t),
+               (-t, t, -t), (0.6, 0.8, 0), (0, 0, 0), (1e-30, 0.6, 0.8), (1e-20, 1e-20, 1),
+               (1e-38, 1e-38, 1), (3e-39, 0.6, 0.8), (2.0, 0.0, 0.0), (0.3, 0.4, 1.2)]
+    vols = [0.0, 0.5, 1.0, 1e-7, 1 - 1e-7, 1e-30, 0.25, 0.75, 1.0 / 6.0, -0.5, 1.5]
+    n = np.array([nn for nn in normals for _ in vols], dtype=np.float32)
+    V0 = np.array([v for _ in normals for v in vols], dtype=np.float32)
+    nx, ny, nz = n[:, 0].copy(), n[:, 1].copy(), n[:, 2].copy()
+    ref = oracle.solve(V0, nx, ny, nz)              # oracle: V0<0 -> -S/2, V0>1 -> +S/2, n=0 -> 0
+    tV, tx, ty, tz = dev(V0, nx, ny, nz)
+    got = plic.plic_solve(tV, tx, ty, tz, method=method, fast=fast).cpu().numpy()
+    assert np.all(np.isfinite(got))
+    assert np.max(np.abs(got.astype(np.float64) - ref)) <= TOL_D0
+    zero = (n == 0).all(1)
+    assert np.all(got[zero] == 0.0)
+
+
+def test_homogeneity_and_method_agreement(plic):
+    V0, nx, ny, nz = gen.random_sphere(1 << 18, seed=21)
+    tV, tx, ty, tz = dev(V0, nx, ny, nz)
+    base = {}
+    for method, fast in VARIANTS:
+        d = plic.plic_solve(tV, tx, ty, tz, method=method, fast=fast)
+        base[(method, fast)] = d
+        for lam in (0.5, 4.0):                      # exact powers of two: d0(V0, c n) = c d0(V0, n)
+            dl = plic.plic_solve(tV, tx * lam, ty * lam, tz * lam, method=method, fast=fast)
+            assert float((dl - lam * d).abs().max()) <= 2e-5 * lam, (method, fast, lam)
+    # "apart from floating-point errors, the SZ solution and our own produce identical
+    # results"
+    assert float((base[("analytic", False)] - base[("sz", False)]).abs().max()) <= 5e-6
+    for key, d in base.items():
+        assert float((d - base[("analytic", False)]).abs().max()) <= 2e-5, key
+
+
+# ------------------------------------------------------------------------------------------
+# forward map
+# ------------------------------------------------------------------------------------------
+def test_volume_parity(plic):
+    V0, nx, ny, nz = gen.config1(seed=0)
+    S = (np.abs(nx) + np.abs(ny) + np.abs(nz)).astype(np.float64)
+    rng = np.random.default_rng(7)
+    d0 = ((rng.random(V0.shape[0]) - 0.5) * S * 1.05).astype(np.float32)   # some planes miss the cube
+    ref = oracle.volume(d0, nx, ny, nz)
+    td, tx, ty, tz = dev(d0, nx, ny, nz)
+    got = plic.plic_volume(td, tx, ty, tz).cpu().numpy()
+    assert np.all(np.isfinite(got)) and got.min() >= 0.0 and got.max() <= 1.0
+    assert np.max(np.abs(got.astype(np.float64) - ref)) <= TOL_VOL
+    # ragged sizes and the zero normal
+    for N in (1, 3, 5, 1027):
+        g = plic.plic_volume(td[:N], tx[:N], ty[:N], tz[:N]).cpu().numpy()
+        assert np.max(np.abs(g.astype(np.float64) - ref[:N])) <= TOL_VOL
+    z = torch.zeros(3, device="cuda")
+    g = plic.plic_volume(torch.tensor([-0.1, 0.0, 0.1], device="cuda"), z, z, z).cpu().numpy()
+    assert g.tolist() == [0.0, 0.5, 1.0]
+
+
+def test_volume_small_n1(plic):
+    rng = np.random.default_rng(5)
+    m = 1 << 17
+    n1 = 10.0 ** rng.uniform(-12, -0.5, m)
+    ang = rng.uniform(0, 2 * np.pi, m)
+    g = np.stack([np.cos(ang), n1, np.sin(ang)], 1)
+    g = (g / np.linalg.norm(g, axis=1, keepdims=True)).astype(np.float32)
+    S = np.abs(g.astype(np.float64)).sum(1)
+    d0 = ((rng.random(m) - 0.5) * S).astype(np.float32)
+    ref = oracle.volume(d0, g[:, 0], g[:, 1], g[:, 2])
+    td, tx, ty, tz = dev(d0, g[:, 0], g[:, 1], g[:, 2])
+    got = plic.plic_volume(td, tx, ty, tz).cpu().numpy()
+    assert np.max(np.abs(got.astype(np.float64) - ref)) <= TOL_VOL
+
+
+# ------------------------------------------------------------------------------------------
+# host-array API (the e2e path of bench.py)
+# ------------------------------------------------------------------------------------------
+def test_host_api_matches_device_api_bitwise(plic):
+    N = (1 << 23) + 12345            # spans three pipeline chunks and a ragged tail
+    V0, nx, ny, nz = gen.random_sphere(N, seed=31)
+    tV, tx, ty, tz = dev(V0, nx, ny, nz)
+    for method, fast in (("analytic", True), ("sz", False)):
+        want = plic.plic_solve(tV, tx, ty, tz, method=method, fast=fast).cpu().numpy()
+        got = plic.plic_solve_host(V0, nx, ny, nz, method=method, fast=fast)       # pageable numpy
+        assert np.array_equal(got, want)
+        pin = [torch.from_numpy(a).pin_memory() for a in (V0, nx, ny, nz)]
+        out = torch.empty(N, dtype=torch.float32).pin_memory()
+        plic.plic_solve_host(*pin, out=out, method=method, fast=fast)              # pinned torch
+        assert np.array_equal(out.numpy(), want)
+    d0 = plic.plic_solve(tV, tx, ty, tz).cpu().numpy()
+    want = plic.plic_volume(*dev(d0, nx, ny, nz)).cpu().numpy()
+    assert np.array_equal(plic.plic_volume_host(d0, nx, ny, nz), want)
+    plic.plic_host_release()
+    assert np.array_equal(plic.plic_volume_host(d0[:1000], nx[:1000], ny[:1000], nz[:1000]), want[:1000])
+
+
+def test_non_default_stream(plic):
+    V0, nx, ny, nz = gen.random_sphere(100000, seed=41)
+    tV, tx, ty, tz = dev(V0, nx, ny, nz)
+    want = plic.plic_solve(tV, tx, ty, tz, method="sz")
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        got = plic.plic_solve(tV, tx, ty, tz, method="sz")
+    s.synchronize()
+    assert torch.equal(got, want)
+
+
+# ------------------------------------------------------------------------------------------
+# full size, in the launch configuration bench.py times: 2^26 cells, seed 1; every 64th cell
+# checked against the oracle, plus properties that hold at any size
+# ------------------------------------------------------------------------------------------
+def test_full_size_config2_sampled(plic):
+    N = 1 << 26
+    V0, nx, ny, nz = gen.random_sphere(N, seed=1)
+    tV, tx, ty, tz = dev(V0, nx, ny, nz)
+    sl = slice(5, None, 64)
+    ref = oracle.solve(V0[sl], nx[sl], ny[sl], nz[sl])
+    S2 = 0.5 * (tx.abs() + ty.abs() + tz.abs())
+    out = torch.empty_like(tV)
+    for method, fast in VARIANTS:
+        grid, block, cpt = plic.plic_launch_config(method, N, fast)
+        assert block == 256 and cpt == 4 and grid % 148 == 0
+        plic.plic_solve(tV, tx, ty, tz, out=out, method=method, fast=fast)
+        assert bool(torch.isfinite(out).all())
+        assert bool((out.abs() <= S2 * (1 + 1e-6)).all())
+        assert bool((torch.sign(out) * torch.sign(tV - 0.5) >= 0).all())       # eq. (8)
+        got = out[sl].cpu().numpy().astype(np.float64)
+        assert np.max(np.abs(got - ref)) <= TOL_D0, (method, fast)
+        back = plic.plic_volume(out, tx, ty, tz)
+        assert float((back - tV).abs().max()) <= 2e-5                          # eq. (31)
+
+
+# ------------------------------------------------------------------------------------------
+# config 5: sphere of radius 60 on a 256^3 lattice
+# ------------------------------------------------------------------------------------------
+def test_sphere_lattice(plic):
+    s = gen.sphere_lattice()
+    phi, nx, ny, nz, r = s["phi"], s["nx"], s["ny"], s["nz"], s["r"]
+    assert 55000 < phi.shape[0] < 65000
+    ref = oracle.solve(phi, nx, ny, nz)
+    dev_ref = np.abs(r + ref - 60.0)                # distance of the oracle's plane from the centre
+    for method, fast in VARIANTS:
+        got, _ = check_solve(plic, phi, nx, ny, nz, method, fast, ref, "sphere")
+        dev_gpu = np.abs(r + got.astype(np.float64) - 60.0)
+        # the reconstructed planes are as close to the sphere as the exact solver's: the
+        # statistic is a property of the 8^3 fill-level sampler, not of the solver
+        assert abs(dev_gpu.max() - dev_ref.max()) <= 4e-5
+        assert abs(dev_gpu.mean() - dev_ref.mean()) <= 1e-5
+        assert np.quantile(dev_gpu, 0.999) <= 0.05
+        # BASELINE.json's literal "<= 0.05 cell" bound is exceeded by the exact fp64 solve on
+        # a handful of nearly axis-aligned cells; the GPU must not add to them
+        n_ref = int((dev_ref > 0.05).sum())
+        assert n_ref <= 8
+        assert (dev_gpu > 0.05 + 4e-5).sum() <= n_ref <= (dev_gpu > 0.05 - 4e-5).sum()
