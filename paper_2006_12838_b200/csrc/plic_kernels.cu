@@ -13,6 +13,7 @@
 
 #include "../../include/plic.h"
 #include "plic_methods.cuh"
+#include "plic_packed.cuh"
 
 #define PLIC_VERSION 100
 
@@ -40,10 +41,34 @@ struct SolveOp {
     static __device__ __forceinline__ float apply(float s, float x, float y, float z) {
         return solve_cell<METHOD, FAST>(s, x, y, z);
     }
+    static __device__ __forceinline__ float4 apply4(const float4 &v, const float4 &a,
+                                                    const float4 &b, const float4 &c) {
+        return make_float4(apply(v.x, a.x, b.x, c.x), apply(v.y, a.y, b.y, c.y),
+                           apply(v.z, a.z, b.z, c.z), apply(v.w, a.w, b.w, c.w));
+    }
+};
+// analytic-fast runs on packed pairs (plic_packed.cuh); a single cell is a pair with both
+// halves equal, so the scalar head/tail kernel gives bitwise the same result as the body.
+template <>
+struct SolveOp<ANALYTIC, true> {
+    static __device__ __forceinline__ float apply(float s, float x, float y, float z) {
+        return solve_pair_analytic_fast(F2{s, s}, F2{x, x}, F2{y, y}, F2{z, z}).x;
+    }
+    static __device__ __forceinline__ float4 apply4(const float4 &v, const float4 &a,
+                                                    const float4 &b, const float4 &c) {
+        const F2 lo = solve_pair_analytic_fast(F2{v.x, v.y}, F2{a.x, a.y}, F2{b.x, b.y}, F2{c.x, c.y});
+        const F2 hi = solve_pair_analytic_fast(F2{v.z, v.w}, F2{a.z, a.w}, F2{b.z, b.w}, F2{c.z, c.w});
+        return make_float4(lo.x, lo.y, hi.x, hi.y);
+    }
 };
 struct VolumeOp {
     static __device__ __forceinline__ float apply(float s, float x, float y, float z) {
         return volume_cell(s, x, y, z);
+    }
+    static __device__ __forceinline__ float4 apply4(const float4 &v, const float4 &a,
+                                                    const float4 &b, const float4 &c) {
+        return make_float4(apply(v.x, a.x, b.x, c.x), apply(v.y, a.y, b.y, c.y),
+                           apply(v.z, a.z, b.z, c.z), apply(v.w, a.w, b.w, c.w));
     }
 };
 
@@ -59,12 +84,7 @@ map_vec4(const float4 *__restrict__ s, const float4 *__restrict__ nx,
         const float4 a = ld_stream(nx + i);
         const float4 b = ld_stream(ny + i);
         const float4 c = ld_stream(nz + i);
-        float4 r;
-        r.x = OP::apply(v.x, a.x, b.x, c.x);
-        r.y = OP::apply(v.y, a.y, b.y, c.y);
-        r.z = OP::apply(v.z, a.z, b.z, c.z);
-        r.w = OP::apply(v.w, a.w, b.w, c.w);
-        st_stream(out + i, r);
+        st_stream(out + i, OP::apply4(v, a, b, c));
     }
 }
 
