@@ -1,8 +1,8 @@
-"""Derives the polynomial coefficients hard-coded in plic_math.cuh (run by hand; prints them).
+"""Derives the polynomial coefficients hard-coded in plic_packed.cuh (run by hand; prints them).
 
-  sin_third_asin_fast:  g(C) = sin(asin(C)/3) ~ C * P3(C^2) on [0, 0.9], then one Newton step
+  neg_sin_third_asin_fast2: g(C) = sin(asin(C)/3) ~ C * P3(C^2) on [0, 0.9], then one Newton step
                         on 3g - 4g^3 = C.
-  acos_fast:            acos(x) ~ sqrt(1-x) * Q(x) on [0, 1].
+  acos_fast2:           acos(x) ~ sqrt(1-x) * Q(x) on [0, 1].
 
 Weighted least squares on Chebyshev nodes with Lawson re-weighting (converges to the minimax
 fit).  Part of the CUDA path's sources; nothing under oracle/ or tests/ uses it.

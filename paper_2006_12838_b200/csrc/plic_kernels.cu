@@ -1,10 +1,17 @@
 // plic_kernels.cu -- kernels, launch logic and the C ABI of libplic (include/plic.h).
 //
 // One elementwise pass per call: 16 B read + 4 B written per cell, no reuse, so the kernels
-// are built around HBM streaming: 128-bit loads of four SoA arrays (one float4 = 4 cells per
-// array per thread), L1 no-allocate, a persistent grid of (SM count x resident blocks)
-// thread blocks striding over the array, 128-bit stores.  Not a contraction: no tensor
-// cores, no shared-memory staging (each byte is used exactly once by exactly one thread).
+// are built around HBM streaming over a persistent grid of (SM count x resident blocks)
+// thread blocks striding over the arrays, one float4 (4 cells) per array per thread per
+// step, 128-bit streaming stores.  Two bodies:
+//   map_tma   the HBM-bound PLIC_FAST kernels (analytic, SZ, Newton): the four input tiles of
+//             a step are brought into shared memory by 1-D bulk asynchronous copies
+//             (cp.async.bulk, SASS UBLKCP) signalled on an mbarrier, kStages tiles ahead of
+//             the arithmetic, so the bytes in flight per SM are set by shared memory
+//             (4 blocks x 3 stages x 16 KB) and not by registers x occupancy;
+//   map_vec4  every other kernel (bound by instruction issue): direct 128-bit
+//             ld.global.nc.L1::no_allocate loads.
+// Not a contraction: no tensor cores.  Each byte is used exactly once by exactly one thread.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -38,6 +45,8 @@ __device__ __forceinline__ void st_stream(float4 *p, const float4 &v) {
 // op(V0-or-d0, nx, ny, nz) -> result, for one cell
 template <int METHOD, bool FAST>
 struct SolveOp {
+    static constexpr int kMinBlocks = 0;      // resident blocks per SM asked of ptxas; 0 = its choice
+    static constexpr bool kTma = false;       // body kernel: map_vec4
     static __device__ __forceinline__ float apply(float s, float x, float y, float z) {
         return solve_cell<METHOD, FAST>(s, x, y, z);
     }
@@ -47,34 +56,43 @@ struct SolveOp {
                            apply(v.z, a.z, b.z, c.z), apply(v.w, a.w, b.w, c.w));
     }
 };
-// analytic-fast runs on packed pairs (plic_packed.cuh); a single cell is a pair with both
-// halves equal, so the scalar head/tail kernel gives bitwise the same result as the body.
-template <>
-struct SolveOp<ANALYTIC, true> {
+// The PLIC_FAST variants run on packed pairs (plic_packed.cuh); a single cell is a pair with
+// both halves equal, so the scalar head/tail kernel gives bitwise the same result as the body.
+template <int METHOD>
+struct SolveOp<METHOD, true> {
+    // nested intervals is bound by instruction issue and stays on map_vec4 at 6 blocks per SM
+    // (40 registers); the other three are staged through shared memory (map_tma) at 4 blocks
+    // per SM (64 registers, 4 x 48 KB of stages)
+    static constexpr bool kTma = METHOD != NESTED;
+    static constexpr int kMinBlocks = kTma ? 4 : 6;
     static __device__ __forceinline__ float apply(float s, float x, float y, float z) {
-        return solve_pair_analytic_fast(F2{s, s}, F2{x, x}, F2{y, y}, F2{z, z}).x;
+        return solve_pair_fast<METHOD>(F2{s, s}, F2{x, x}, F2{y, y}, F2{z, z}).x;
     }
     static __device__ __forceinline__ float4 apply4(const float4 &v, const float4 &a,
                                                     const float4 &b, const float4 &c) {
-        const F2 lo = solve_pair_analytic_fast(F2{v.x, v.y}, F2{a.x, a.y}, F2{b.x, b.y}, F2{c.x, c.y});
-        const F2 hi = solve_pair_analytic_fast(F2{v.z, v.w}, F2{a.z, a.w}, F2{b.z, b.w}, F2{c.z, c.w});
+        const F2 lo = solve_pair_fast<METHOD>(F2{v.x, v.y}, F2{a.x, a.y}, F2{b.x, b.y}, F2{c.x, c.y});
+        const F2 hi = solve_pair_fast<METHOD>(F2{v.z, v.w}, F2{a.z, a.w}, F2{b.z, b.w}, F2{c.z, c.w});
         return make_float4(lo.x, lo.y, hi.x, hi.y);
     }
 };
+// plic_volume also runs on packed pairs, branch-free, one division per cell (volume_pair).
 struct VolumeOp {
+    static constexpr bool kTma = true;
+    static constexpr int kMinBlocks = 4;
     static __device__ __forceinline__ float apply(float s, float x, float y, float z) {
-        return volume_cell(s, x, y, z);
+        return volume_pair(F2{s, s}, F2{x, x}, F2{y, y}, F2{z, z}).x;
     }
     static __device__ __forceinline__ float4 apply4(const float4 &v, const float4 &a,
                                                     const float4 &b, const float4 &c) {
-        return make_float4(apply(v.x, a.x, b.x, c.x), apply(v.y, a.y, b.y, c.y),
-                           apply(v.z, a.z, b.z, c.z), apply(v.w, a.w, b.w, c.w));
+        const F2 lo = volume_pair(F2{v.x, v.y}, F2{a.x, a.y}, F2{b.x, b.y}, F2{c.x, c.y});
+        const F2 hi = volume_pair(F2{v.z, v.w}, F2{a.z, a.w}, F2{b.z, b.w}, F2{c.z, c.w});
+        return make_float4(lo.x, lo.y, hi.x, hi.y);
     }
 };
 
 // Body: n4 float4 groups (4 cells each), grid-stride.
 template <class OP>
-__global__ void __launch_bounds__(kBlock)
+__global__ void __launch_bounds__(kBlock, OP::kMinBlocks)
 map_vec4(const float4 *__restrict__ s, const float4 *__restrict__ nx,
          const float4 *__restrict__ ny, const float4 *__restrict__ nz,
          float4 *__restrict__ out, int64_t n4) {
@@ -85,6 +103,103 @@ map_vec4(const float4 *__restrict__ s, const float4 *__restrict__ nx,
         const float4 b = ld_stream(ny + i);
         const float4 c = ld_stream(nz + i);
         st_stream(out + i, OP::apply4(v, a, b, c));
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// map_tma: the same map with the input tiles staged through shared memory by the bulk-copy
+// engine.  A tile is kBlock float4 groups (1024 cells) of each of the four arrays = 16 KB;
+// kStages tiles per block are in flight.  Thread 0 arms full[stage] with the byte count and
+// issues four cp.async.bulk; every thread waits on the barrier's phase, copies its float4s
+// to registers, and after a block barrier (all reads of the stage done) thread 0 refills the
+// stage with the tile kStages steps ahead while the block does the arithmetic and stores.
+// ---------------------------------------------------------------------------------------
+constexpr int kStages = 3;
+constexpr int kTileBytes = kBlock * 16;                              // one array's tile
+constexpr int kTmaSmem = kStages * 4 * kTileBytes + kStages * 8;     // stages + mbarriers
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+            smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+
+template <class OP>
+__global__ void __launch_bounds__(kBlock, OP::kMinBlocks)
+map_tma(const float4 *__restrict__ s, const float4 *__restrict__ nx,
+        const float4 *__restrict__ ny, const float4 *__restrict__ nz,
+        float4 *__restrict__ out, int64_t n4) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float4 *buf = reinterpret_cast<float4 *>(smem_raw);              // [kStages][4][kBlock]
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + kStages * 4 * kTileBytes);
+    const int tid = threadIdx.x;
+    const int64_t ntiles = (n4 + kBlock - 1) / kBlock;
+    const int64_t first = blockIdx.x, step = gridDim.x;
+
+    auto issue = [&](int64_t tile, int stage) {                      // thread 0 only
+        const int64_t base = tile * kBlock;
+        const int64_t rem = n4 - base;
+        const uint32_t bytes = (uint32_t)(rem < kBlock ? rem : kBlock) * 16u;   // ragged last tile
+        float4 *dst = buf + stage * 4 * kBlock;
+        mbar_expect_tx(&full[stage], 4 * bytes);
+        bulk_g2s(dst, s + base, bytes, &full[stage]);
+        bulk_g2s(dst + kBlock, nx + base, bytes, &full[stage]);
+        bulk_g2s(dst + 2 * kBlock, ny + base, bytes, &full[stage]);
+        bulk_g2s(dst + 3 * kBlock, nz + base, bytes, &full[stage]);
+    };
+    if (tid == 0) {
+        for (int k = 0; k < kStages; ++k) mbar_init(&full[k], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        for (int k = 0; k < kStages; ++k)
+            if (first + k * step < ntiles) issue(first + k * step, k);
+    }
+    __syncthreads();                                                 // barriers initialised
+    int stage = 0;
+    uint32_t parity = 0;
+    for (int64_t tile = first; tile < ntiles; tile += step) {
+        mbar_wait(&full[stage], parity);
+        const float4 *src = buf + stage * 4 * kBlock;
+        // in a ragged last tile the slots past the end hold stale data of an earlier tile
+        // (or nothing): they are computed and dropped, never stored
+        const float4 v = src[tid], a = src[kBlock + tid], b = src[2 * kBlock + tid],
+                     c = src[3 * kBlock + tid];
+        __syncthreads();                                             // stage fully read
+        if (tid == 0) {
+            const int64_t next = tile + kStages * step;
+            if (next < ntiles) issue(next, stage);
+        }
+        const int64_t i = tile * kBlock + tid;
+        if (i < n4) st_stream(out + i, OP::apply4(v, a, b, c));
+        if (++stage == kStages) {
+            stage = 0;
+            parity ^= 1;
+        }
     }
 }
 
@@ -122,17 +237,29 @@ typedef void (*vec_kernel_t)(const float4 *, const float4 *, const float4 *, con
 typedef void (*scalar_kernel_t)(const float *, const float *, const float *, const float *,
                                 float *, int64_t, int64_t, int64_t);
 
-static vec_kernel_t vec_kernel(int k) {
+// body kernel of an op and the dynamic shared memory it needs
+struct BodyKernel {
+    vec_kernel_t fn;
+    int smem;
+};
+template <class OP>
+static BodyKernel body_of() {
+    if constexpr (OP::kTma)
+        return BodyKernel{map_tma<OP>, kTmaSmem};
+    else
+        return BodyKernel{map_vec4<OP>, 0};
+}
+static BodyKernel vec_kernel(int k) {
     switch (k) {
-        case 0: return map_vec4<SolveOp<ANALYTIC, false>>;
-        case 1: return map_vec4<SolveOp<SZ, false>>;
-        case 2: return map_vec4<SolveOp<NEWTON, false>>;
-        case 3: return map_vec4<SolveOp<NESTED, false>>;
-        case 4: return map_vec4<SolveOp<ANALYTIC, true>>;
-        case 5: return map_vec4<SolveOp<SZ, true>>;
-        case 6: return map_vec4<SolveOp<NEWTON, true>>;
-        case 7: return map_vec4<SolveOp<NESTED, true>>;
-        default: return map_vec4<VolumeOp>;
+        case 0: return body_of<SolveOp<ANALYTIC, false>>();
+        case 1: return body_of<SolveOp<SZ, false>>();
+        case 2: return body_of<SolveOp<NEWTON, false>>();
+        case 3: return body_of<SolveOp<NESTED, false>>();
+        case 4: return body_of<SolveOp<ANALYTIC, true>>();
+        case 5: return body_of<SolveOp<SZ, true>>();
+        case 6: return body_of<SolveOp<NEWTON, true>>();
+        case 7: return body_of<SolveOp<NESTED, true>>();
+        default: return body_of<VolumeOp>();
     }
 }
 static scalar_kernel_t scalar_kernel(int k) {
@@ -168,8 +295,13 @@ static DeviceInfo *device_info(cudaError_t *err) {
     std::call_once(info->once, [info, dev]() {
         cudaError_t e2 = cudaDeviceGetAttribute(&info->sms, cudaDevAttrMultiProcessorCount, dev);
         for (int k = 0; k < kNumKernels && e2 == cudaSuccess; ++k) {
-            e2 = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&info->blocks_per_sm[k],
-                                                               vec_kernel(k), kBlock, 0);
+            const BodyKernel body = vec_kernel(k);
+            if (body.smem > 0)
+                e2 = cudaFuncSetAttribute(body.fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          body.smem);
+            if (e2 == cudaSuccess)
+                e2 = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&info->blocks_per_sm[k], body.fn,
+                                                                   kBlock, body.smem);
             if (info->blocks_per_sm[k] < 1) info->blocks_per_sm[k] = 1;
         }
         info->err = e2;
@@ -207,7 +339,8 @@ static int launch_map(int k, const float *s, const float *nx, const float *ny, c
     const int64_t tail0 = head + 4 * n4;
 
     if (n4 > 0) {
-        vec_kernel(k)<<<grid_for(info, k, n4), kBlock, 0, stream>>>(
+        const BodyKernel body = vec_kernel(k);
+        body.fn<<<grid_for(info, k, n4), kBlock, body.smem, stream>>>(
             (const float4 *)(s + head), (const float4 *)(nx + head), (const float4 *)(ny + head),
             (const float4 *)(nz + head), (float4 *)(out + head), n4);
         g_launches.fetch_add(1, std::memory_order_relaxed);

@@ -9,8 +9,11 @@
 //   n12 = n1+n2, S = n1+n2+n3, q = n1 n2, W = 2 V n3, z = n12 - W, e = n3 - n12,
 //   x = 6 V n2 n3 = 3 W n2,  u = 4 q - e^2  ( = S^2 - 2 sum n_i^2; = t4/9 of eq. (19) when |n|=1 ).
 //
-// Each method is `reduced_offset<METHOD, FAST>(n1, n2, n3, V) -> d`; the frame solve_cell()
-// does the symmetry reduction before and the sign restore (eq. (8)) after.  The bodies of
+// This file holds the precise (FAST = false) kernels: IEEE division and square root, CUDA
+// libm cbrt/asin/acos/sin/cos, branches in the paper's order.  The PLIC_FAST kernels are in
+// plic_packed.cuh (two cells per instruction, branch-free, SFU roots); cbrt_seed() here
+// serves both.  Each method is `Solver<METHOD, false>::reduced_offset(n1, n2, n3, V) -> d`; the
+// frame solve_cell() does the symmetry reduction before and the sign restore (eq. (8)) after.  The bodies of
 // the paper's Listings 1, 2, 4, 5, 6 are not in PAPER.md (captions only) and Listing 3 is
 // truncated, so every method is built from the equations; DESIGN.md lists the readings.
 //
@@ -99,43 +102,6 @@ struct Solver<ANALYTIC, false> {
     }
 };
 
-// One trigonometric evaluation serving (3) and (4): parameters selected, then evaluated once.
-template <bool FAST>
-__device__ __forceinline__ float trig_case34(float n1, float n2, float n3, float n12, float W) {
-    const float q = n1 * n2;
-    const float e = n3 - n12;
-    const float z = n12 - W;
-    const float ee = e * e;
-    const bool c4 = is_case4(q, e, ee, z);
-    const float u = fmaf(4.0f, q, -ee);
-    const float X = c4 ? u : q + q;
-    const float r = mufu_rsqrt(X);
-    const float Xr = X * r;                                   // sqrt(X)
-    const float K = c4 ? 6.0f * q * (n3 - W) * (r * r) : 0.75f * z;
-    const float g = Math<FAST>::sin_third_asin(K * r);
-    const float B = c4 ? Xr : Xr + Xr;
-    const float A = c4 ? 0.5f * (n12 + n3) : n12;
-    return fmaxf(fmaf(-B, g, A), c4 ? n3 : n2);               // bracket floor; also drops NaN
-}
-
-// Fast: every closed form evaluated, merged by select; (3)/(4) share one trig evaluation.
-template <>
-struct Solver<ANALYTIC, true> {
-    static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
-        typedef Math<true> M;
-        const float n12 = n1 + n2;
-        const float W = (V + V) * n3;
-        const float x = 3.0f * W * n2;
-        const float s1 = n1 * n1;
-        const bool c5 = n12 <= W;
-        const float d2 = fmaf(0.5f, n1, M::sqrt(fmaxf(fmaf(W, n2, -s1 * (1.0f / 12.0f)), 0.0f)));
-        const float d1 = M::cbrt(x * n1);
-        float d = x < s1 ? d1 : d2;
-        if (!c5 && x > fmaf(3.0f * n2, n2 - n1, s1)) d = trig_case34<true>(n1, n2, n3, n12, W);
-        return c5 ? 0.5f * (W + n12) : d;
-    }
-};
-
 // ---------------------------------------------------------------------------------------
 // method 1: Scardovelli-Zaleski, edge-case complete and micro-optimised (sect. 2.4)
 //
@@ -153,10 +119,10 @@ struct Solver<ANALYTIC, true> {
 // -- the literal a2, a1, a0 arithmetic loses all significance in fp32 when m1 is small
 // ("SZ cancellation").
 // ---------------------------------------------------------------------------------------
-template <bool FAST>
-struct Solver<SZ, FAST> {
+template <>
+struct Solver<SZ, false> {
     static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
-        typedef Math<FAST> M;
+        typedef Math<false> M;
         const float S = (n1 + n2) + n3;
         const float inv = M::div(1.0f, S);
         const float m1 = n1 * inv, m2 = n2 * inv, m3 = n3 * inv;
@@ -234,37 +200,6 @@ struct Solver<NEWTON, false> {
     }
 };
 
-// Fast: one unrolled Newton loop serves (1), (3) and (4) with per-case (p, r, tau0, base).
-template <>
-struct Solver<NEWTON, true> {
-    static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
-        typedef Math<true> M;
-        const float n12 = n1 + n2;
-        const float W = (V + V) * n3;
-        const float x = 3.0f * W * n2;
-        const float s1 = n1 * n1;
-        const bool c5 = n12 <= W;
-        const bool c1 = x < s1;
-        float d = fmaf(0.5f, n1, M::sqrt(fmaxf(fmaf(W, n2, -s1 * (1.0f / 12.0f)), 0.0f)));   // (2)
-        if (!c5 && (c1 || x > fmaf(3.0f * n2, n2 - n1, s1))) {
-            const float q = n1 * n2;
-            const float e = n3 - n12;
-            const float z = n12 - W;
-            const float ee = e * e;
-            const bool c4 = is_case4(q, e, ee, z);
-            const float k = x * n1;
-            float p = c4 ? 0.75f * fmaf(4.0f, q, -ee) : 6.0f * q;
-            float r = c4 ? 1.5f * q * (n3 - W) : 3.0f * q * z;
-            float tau = c4 ? 0.0f : fminf(e, 0.0f);
-            float base = c4 ? 0.5f * (n12 + n3) : n12;
-            float floor_ = c4 ? n3 : n2;
-            if (c1) { p = 0.0f; r = k; tau = cbrt_seed(k); base = 0.0f; floor_ = 0.0f; }
-            d = fmaxf(base + newton_cubic<true, 4>(p, r, tau), floor_);
-        }
-        return c5 ? 0.5f * (W + n12) : d;
-    }
-};
-
 // ---------------------------------------------------------------------------------------
 // method 3: nested intervals (bisection) for cases (3), (4); closed forms otherwise (sect. 2.5)
 // F is decreasing on the bracket [lo, hi] with F(lo) >= 0 >= F(hi).
@@ -281,24 +216,10 @@ __device__ __forceinline__ float bisect_cubic_converged(float p, float r, float 
     return 0.5f * (lo + hi);
 }
 
-// Fast: a fixed number of halvings, branch-free (lo, width) form.
-template <int HALVINGS>
-__device__ __forceinline__ float bisect_cubic_fixed(float p, float r, float lo, float hi) {
-    float w = hi - lo;
-#pragma unroll
-    for (int i = 0; i < HALVINGS; ++i) {
-        w *= 0.5f;
-        const float mid = lo + w;
-        const float F = fmaf(fmaf(mid, mid, -p), mid, -r);
-        lo = F > 0.0f ? mid : lo;
-    }
-    return fmaf(0.5f, w, lo);
-}
-
-template <bool FAST>
-struct Solver<NESTED, FAST> {
+template <>
+struct Solver<NESTED, false> {
     static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
-        typedef Math<FAST> M;
+        typedef Math<false> M;
         const float n12 = n1 + n2;
         const float W = 2.0f * V * n3;
         const bool c5 = n12 <= W;
@@ -321,8 +242,7 @@ struct Solver<NESTED, FAST> {
             const float r = c4 ? 1.5f * q * (n3 - W) : 3.0f * q * z;
             const float lo = c4 ? n3 - hS : -n1;
             const float hi = c4 ? 0.0f : fminf(e, 0.0f);
-            const float tau = FAST ? bisect_cubic_fixed<20>(p, r, lo, hi)
-                                   : bisect_cubic_converged(p, r, lo, hi);
+            const float tau = bisect_cubic_converged(p, r, lo, hi);
             d = (c4 ? hS : n12) + tau;
         }
         return c5 ? fmaf(V, n3, 0.5f * n12) : d;

@@ -72,8 +72,14 @@ __device__ __forceinline__ F2 rcp2(F2 a) { return F2{mufu_rcp(a.x), mufu_rcp(a.y
 __device__ __forceinline__ F2 lg2_2(F2 a) { return F2{mufu_lg2(a.x), mufu_lg2(a.y)}; }
 __device__ __forceinline__ F2 ex2_2(F2 a) { return F2{mufu_ex2(a.x), mufu_ex2(a.y)}; }
 
-// -sin(asin(C)/3), both halves: sin_third_asin_fast() of plic_math.cuh on a pair, negated
-// (the Newton step's denominator is taken with the opposite sign, which costs nothing)
+// -sin(asin(C)/3) for C in [0, 0.9], both halves.  g = sin(asin(C)/3) is the root in [0, 0.36]
+// of the triple-angle relation 3g - 4g^3 = C.  An odd minimax start value C*P3(C^2)
+// (|err| < 2.0e-4 on [0, 0.9]) is polished by one Newton step g <- (C - 8g^3)/(3 - 12g^2),
+// whose denominator stays >= 1.4; the result is within 1.3e-7 of the exact value.  This
+// replaces the asin + sin pair of the trigonometric cubic root (eq. (12)): the
+// argument range C <= 5/(4 sqrt 2) = 0.884 is a property of cases (3)/(4) ("trig
+// range").  The step's denominator is taken with the opposite sign, which negates the result
+// at no cost.  Coefficients: fit_coefficients.py.
 __device__ __forceinline__ F2 neg_sin_third_asin_fast2(F2 C) {
     const F2 C2 = mul2(C, C);
     F2 g = fma2(C2, f2(0.100619423f), f2(-0.0602495379f));
@@ -86,57 +92,299 @@ __device__ __forceinline__ F2 neg_sin_third_asin_fast2(F2 C) {
     return mul2(num, rcp2(den));
 }
 
+__device__ __forceinline__ F2 cos2(F2 a) { return F2{mufu_cos(a.x), mufu_cos(a.y)}; }
+__device__ __forceinline__ F2 sat2(F2 a) { return F2{__saturatef(a.x), __saturatef(a.y)}; }
+__device__ __forceinline__ F2 abs2(F2 a) { return F2{fabsf(a.x), fabsf(a.y)}; }
+
 // ---------------------------------------------------------------------------------------
-// analytic inverse (eq. (25)/(26)), PLIC_FAST, for two cells at once.  Same arithmetic as
-// Solver<ANALYTIC, true> was in round 1 -- every closed form evaluated and merged by select,
-// (3)/(4) chosen a priori and served by one trigonometric evaluation -- but with no branch
-// at all, so that the two cells of a pair (and the 32 lanes of a warp) share one instruction
-// stream.  With R = 8 q (case 3) or u (case 4) and rho = rsqrt(R):
+// frame for a pair: symmetry reduction in (eq. (2)-(5)), sign restore out (eq. (8))
+// ---------------------------------------------------------------------------------------
+struct PairIn {
+    F2 n1, n2, n3;   // sorted |n|, eq. (2)-(4)
+    F2 n12;          // n1 + n2
+    F2 hS;           // S/2
+    F2 V2;           // 2 V = 2 min(V0, 1 - V0), saturated to [0, 1]
+};
+
+__device__ __forceinline__ PairIn pair_reduce(F2 V0, F2 nx, F2 ny, F2 nz) {
+    PairIn in;
+    const F2 a = abs2(nx), b = abs2(ny), c = abs2(nz);
+    in.n1 = F2{min3(a.x, b.x, c.x), min3(a.y, b.y, c.y)};                       // eq. (2)
+    in.n3 = F2{max3(a.x, b.x, c.x), max3(a.y, b.y, c.y)};                       // eq. (3)
+    in.n2 = max2(min2(a, b), min2(max2(a, b), c));                              // eq. (4): median
+    // eq. (5): V = 1/2 - |V0 - 1/2| = min(V0, 1 - V0); the saturation makes V0 < 0 act as 0
+    // and V0 > 1 as 1
+    const F2 V = min2(V0, fma2(V0, -1.0f, f2(1.0f)));
+    in.V2 = sat2(add2(V, V));
+    in.n12 = add2(in.n1, in.n2);
+    in.hS = mul2(add2(in.n12, in.n3), 0.5f);
+    return in;
+}
+
+// d0 = sign(V0 - 1/2) (S/2 - d), eq. (8).  d <= S/2 is enforced (also turns a NaN into S/2),
+// so r >= 0 and the sign is a bit operation: set when V0 <= 1/2.
+__device__ __forceinline__ F2 pair_restore(F2 V0, F2 hS, F2 d) {
+    const F2 r = sub2(hS, min2(d, hS));
+    const F2 t = fma2(V0, -1.0f, f2(0.5f));
+    return F2{__uint_as_float(__float_as_uint(r.x) | (~__float_as_uint(t.x) & 0x80000000u)),
+              __uint_as_float(__float_as_uint(r.y) | (~__float_as_uint(t.y) & 0x80000000u))};
+}
+
+// A-priori (3)-vs-(4) decision on a pair: case (4) iff n3 < n12 and F3(e) > 0 (is_case4()).
+__device__ __forceinline__ B2 is_case4_2(F2 q, F2 e, F2 ee, F2 z) {
+    const F2 h = fma2(fma2(q, -6.0f, ee), e, mul2(mul2(q, z), -3.0f));
+    return B2{e.x < 0.0f && h.x > 0.0f, e.y < 0.0f && h.y > 0.0f};
+}
+
+template <int METHOD>
+struct PairSolver;
+
+// ---------------------------------------------------------------------------------------
+// method 0, PLIC_FAST: analytic inverse (eq. (25)/(26)) for two cells at once.  Every closed
+// form is evaluated and merged by select, (3)/(4) are chosen a priori and served by one
+// trigonometric evaluation, and there is no branch at all, so the two cells of a pair (and
+// the 32 lanes of a warp) share one instruction stream.  cbrt = ex2(lg2(x)/3).  With R = 8 q (case 3) or u (case 4) and rho = rsqrt(R):
 //   (3): d = n12 - sqrt(R) g(C),  C = (3/2) z rho           [2 sqrt(2q) = sqrt(8q)]
 //   (4): d = S/2 - sqrt(R) g(C),  C = 6 q (n3 - W) rho^3
 // Both roots are >= n2, which serves as the common floor (it also replaces a NaN from
 // R = 0, i.e. n1 n2 flushed to zero, where the bracket [n2, n12] is narrower than fp32).
 // ---------------------------------------------------------------------------------------
-__device__ __forceinline__ F2 solve_pair_analytic_fast(F2 V0, F2 nx, F2 ny, F2 nz) {
-    const F2 a = F2{fabsf(nx.x), fabsf(nx.y)}, b = F2{fabsf(ny.x), fabsf(ny.y)},
-             c = F2{fabsf(nz.x), fabsf(nz.y)};
-    const F2 n1 = F2{min3(a.x, b.x, c.x), min3(a.y, b.y, c.y)};                 // eq. (2)
-    const F2 n3 = F2{max3(a.x, b.x, c.x), max3(a.y, b.y, c.y)};                 // eq. (3)
-    const F2 n2 = max2(min2(a, b), min2(max2(a, b), c));                        // eq. (4)
-    // eq. (5): V = min(V0, 1 - V0); 2V saturated to [0, 1] (V0 outside [0,1] acts as 0 / 1)
-    const F2 V = min2(V0, fma2(V0, -1.0f, f2(1.0f)));
-    const F2 V2 = F2{__saturatef(V.x + V.x), __saturatef(V.y + V.y)};
+template <>
+struct PairSolver<ANALYTIC> {
+    static __device__ __forceinline__ F2 reduced_offset(const PairIn &in) {
+        const F2 n1 = in.n1, n2 = in.n2, n3 = in.n3, n12 = in.n12;
+        const F2 W = mul2(in.V2, n3);                                           // 2 V n3
+        const F2 Wn2 = mul2(W, n2);                                             // x / 3, x = 6 V n2 n3
+        const F2 s1 = mul2(n1, n1);
+        const F2 t1 = fma2(s1, -1.0f / 3.0f, Wn2);                              // (x - n1^2) / 3
+        // (2) and (1): d1 = cbrt(x n1) = 2^(lg2(Wn2 n1)/3 + lg2(3)/3)
+        const F2 d2 = fma2(n1, 0.5f, sqrt2(max2(fma2(s1, -1.0f / 12.0f, Wn2), 0.0f)));
+        const F2 d1 = ex2_2(fma2(lg2_2(mul2(Wn2, n1)), 1.0f / 3.0f, f2(0.528320834f)));
+        F2 d = sel2(lt2(t1, f2(0.0f)), d1, d2);                                 // x < n1^2
+        // (3)/(4)
+        const F2 q = mul2(n1, n2);
+        const F2 e = sub2(n3, n12);
+        const F2 z = sub2(n12, W);
+        const F2 ee = mul2(e, e);
+        const B2 c4 = is_case4_2(q, e, ee, z);
+        const F2 R = sel2(c4, fma2(q, 4.0f, mul2(ee, -1.0f)), mul2(q, 8.0f));
+        const F2 rho = rsqrt2(R);
+        const F2 K4 = mul2(mul2(mul2(q, 6.0f), sub2(n3, W)), mul2(rho, rho));
+        const F2 C = mul2(sel2(c4, K4, mul2(z, 1.5f)), rho);
+        const F2 ng = neg_sin_third_asin_fast2(C);
+        const F2 d34 = max2(fma2(mul2(R, rho), ng, sel2(c4, in.hS, n12)), n2);  // floor; drops NaN
+        d = sel2(gt2(t1, mul2(n2, sub2(n2, n1))), d34, d);                      // x > n1^2 + 3 n2 (n2 - n1)
+        return sel2(le2(n12, W), mul2(add2(W, n12), 0.5f), d);                  // (5)
+    }
+};
+
+// ---------------------------------------------------------------------------------------
+// method 1, PLIC_FAST: Scardovelli-Zaleski (sect. 2.4) on a pair, branch-free.  Same
+// arithmetic as Solver<SZ, false>, fast roots: L1-normalised m_i = n_i / S, alpha = d / S, thresholds
+// multiplied through, the collapsed p0, q0 (plic_methods.cuh), root
+//   alpha = 2 sqrt(p0) cos(acos(q0 / p0^(3/2)) / 3 + 4 pi / 3) - a2/3
+// with 1/sqrt(p0) from one rsqrt, acos by sqrt(1-x) Q5(x) and cos on the SFU.
+// ---------------------------------------------------------------------------------------
+// acos(x) for x in [0, 1] as sqrt(1-x) * Q5(x), |err| < 1.2e-6 (minimax fit,
+// fit_coefficients.py); the angle is then divided by 3.
+__device__ __forceinline__ F2 acos_fast2(F2 x) {
+    F2 p = fma2(x, f2(-0.004337173733f), f2(0.01934827404f));
+    p = fma2(p, x, f2(-0.04495724702f));
+    p = fma2(p, x, f2(0.08787565452f));
+    p = fma2(p, x, f2(-0.2145122723f));
+    p = fma2(p, x, f2(1.570795206f));
+    return mul2(sqrt2(max2(fma2(x, -1.0f, f2(1.0f)), 0.0f)), p);
+}
+
+template <>
+struct PairSolver<SZ> {
+    static __device__ __forceinline__ F2 reduced_offset(const PairIn &in) {
+        const F2 S = add2(in.n12, in.n3);
+        const F2 inv = rcp2(S);
+        const F2 m1 = mul2(in.n1, inv), m2 = mul2(in.n2, inv), m3 = mul2(in.n3, inv);
+        const F2 m12 = add2(m1, m2);
+        const F2 W = mul2(in.V2, m3);                                           // 2 w m3
+        const F2 Wm2 = mul2(W, m2);
+        const F2 x = mul2(Wm2, 3.0f);                                           // 6 w m2 m3
+        const F2 s1 = mul2(m1, m1);
+        // (2): v1 <= w <= v2, and (1): w < v1  <=>  x < m1^2
+        const F2 a2 = mul2(add2(m1, sqrt2(max2(fma2(s1, -1.0f / 3.0f, mul2(Wm2, 4.0f)), 0.0f))), 0.5f);
+        const F2 a1 = ex2_2(mul2(lg2_2(mul2(x, m1)), 1.0f / 3.0f));             // cbrt(w6)
+        F2 alpha = sel2(lt2(x, s1), a1, a2);
+        // (3)/(4) a priori from v3: case (4) iff m3 < m12 and w6 >= 6 m1 m2 m3 v3
+        const F2 q = mul2(m1, m2);
+        const F2 m3x3 = mul2(m3, 3.0f);
+        F2 v3n = mul2(mul2(m3, m3), fma2(m12, 3.0f, mul2(m3, -1.0f)));
+        v3n = fma2(s1, sub2(m1, m3x3), v3n);
+        v3n = fma2(mul2(m2, m2), sub2(m2, m3x3), v3n);
+        const F2 w6 = mul2(x, m1);
+        const B2 c4 = B2{m3.x < m12.x && w6.x >= v3n.x, m3.y < m12.y && w6.y >= v3n.y};
+        const F2 em = sub2(m12, m3);
+        const F2 p0 = sel2(c4, fma2(mul2(em, -0.25f), em, q), add2(q, q));
+        const F2 q0 = mul2(q, sel2(c4, mul2(sub2(m3, W), 0.75f), mul2(sub2(m12, W), 1.5f)));
+        const F2 rho = rsqrt2(p0);
+        const F2 arg = mul2(mul2(q0, rho), mul2(rho, rho));                     // q0 / p0^(3/2)
+        const F2 theta = mul2(acos_fast2(min2(arg, f2(1.0f))), 1.0f / 3.0f);
+        // cos(theta + 4 pi/3) evaluated as cos(theta - 2 pi/3): same angle, |arg| < pi
+        const F2 co = cos2(add2(theta, f2(-2.0943951f)));
+        const F2 sp2 = mul2(mul2(p0, rho), 2.0f);                               // 2 sqrt(p0)
+        const F2 a34 = max2(fma2(sp2, co, sel2(c4, f2(0.5f), m12)), m2);        // floor; drops NaN
+        alpha = sel2(gt2(x, fma2(mul2(m2, 3.0f), sub2(m2, m1), s1)), a34, alpha);
+        alpha = sel2(le2(m12, W), mul2(add2(W, m12), 0.5f), alpha);             // (5)
+        return mul2(alpha, S);
+    }
+};
+
+// ---------------------------------------------------------------------------------------
+// method 2, PLIC_FAST: Newton-Raphson (sect. 2.5) on a pair.  One unrolled 4-step loop on
+// F(tau) = tau^3 - p tau - r serves (1), (3) and (4) with selected (p, r, tau0, base) -- the
+// start values and trip count of Solver<NEWTON, false>, division by SFU reciprocal; every
+// lane runs it (no branch), (2) and (5) are closed forms.
+// ---------------------------------------------------------------------------------------
+template <>
+struct PairSolver<NEWTON> {
+    static __device__ __forceinline__ F2 reduced_offset(const PairIn &in) {
+        const F2 n1 = in.n1, n2 = in.n2, n3 = in.n3, n12 = in.n12;
+        const F2 W = mul2(in.V2, n3);
+        const F2 Wn2 = mul2(W, n2);
+        const F2 x = mul2(Wn2, 3.0f);
+        const F2 s1 = mul2(n1, n1);
+        const B2 c1 = lt2(x, s1);
+        const F2 d2 = fma2(n1, 0.5f, sqrt2(max2(fma2(s1, -1.0f / 12.0f, Wn2), 0.0f)));
+        const F2 q = mul2(n1, n2);
+        const F2 e = sub2(n3, n12);
+        const F2 z = sub2(n12, W);
+        const F2 ee = mul2(e, e);
+        const B2 c4 = is_case4_2(q, e, ee, z);
+        const F2 k = mul2(x, n1);                                               // 6 V n1 n2 n3
+        const F2 zero = f2(0.0f);
+        F2 p = sel2(c4, mul2(fma2(q, 4.0f, mul2(ee, -1.0f)), 0.75f), mul2(q, 6.0f));
+        F2 r = mul2(q, sel2(c4, mul2(sub2(n3, W), 1.5f), mul2(z, 3.0f)));
+        F2 tau = sel2(c4, zero, min2(e, zero));
+        F2 base = sel2(c4, in.hS, n12);
+        p = sel2(c1, zero, p);
+        r = sel2(c1, k, r);
+        tau = sel2(c1, F2{cbrt_seed(k.x), cbrt_seed(k.y)}, tau);
+        base = sel2(c1, zero, base);
+        const F2 floor_ = sel2(c1, zero, n2);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const F2 t2 = mul2(tau, tau);
+            tau = mul2(fma2(add2(t2, t2), tau, r), rcp2(fma2(t2, 3.0f, mul2(p, -1.0f))));
+        }
+        const F2 dn = max2(add2(base, tau), floor_);                            // floor; drops NaN
+        const F2 thr = fma2(mul2(n2, 3.0f), sub2(n2, n1), s1);
+        const B2 it = B2{c1.x || x.x > thr.x, c1.y || x.y > thr.y};
+        const F2 d = sel2(it, dn, d2);
+        return sel2(le2(n12, W), mul2(add2(W, n12), 0.5f), d);                  // (5)
+    }
+};
+
+// ---------------------------------------------------------------------------------------
+// method 3, PLIC_FAST: nested intervals (sect. 2.5) on a pair: 20 fixed halvings of the
+// bracket of the depressed cubic in branch-free (lo, width) form for (3)/(4) (|err| <= 3e-7;
+// the precise kernel halves until the fp32 midpoint stops moving); closed forms for (1), (2),
+// (5).  F is decreasing on the bracket, F(lo) >= 0.
+// ---------------------------------------------------------------------------------------
+template <>
+struct PairSolver<NESTED> {
+    static __device__ __forceinline__ F2 reduced_offset(const PairIn &in) {
+        const F2 n1 = in.n1, n2 = in.n2, n3 = in.n3, n12 = in.n12;
+        const F2 W = mul2(in.V2, n3);
+        const F2 Wn2 = mul2(W, n2);                                             // x / 3
+        const F2 s1 = mul2(n1, n1);
+        const F2 t1 = fma2(s1, -1.0f / 3.0f, Wn2);                              // (x - n1^2) / 3
+        const F2 d2 = fma2(n1, 0.5f, sqrt2(max2(fma2(s1, -1.0f / 12.0f, Wn2), 0.0f)));
+        const F2 d1 = ex2_2(fma2(lg2_2(mul2(Wn2, n1)), 1.0f / 3.0f, f2(0.528320834f)));
+        F2 d = sel2(lt2(t1, f2(0.0f)), d1, d2);
+        const F2 q = mul2(n1, n2);
+        const F2 e = sub2(n3, n12);
+        const F2 z = sub2(n12, W);
+        const F2 ee = mul2(e, e);
+        const B2 c4 = is_case4_2(q, e, ee, z);
+        const F2 zero = f2(0.0f);
+        const F2 np = sel2(c4, mul2(fma2(q, 4.0f, mul2(ee, -1.0f)), -0.75f), mul2(q, -6.0f));   // -p
+        const F2 nr = mul2(q, sel2(c4, mul2(sub2(n3, W), -1.5f), mul2(z, -3.0f)));              // -r
+        F2 lo = sel2(c4, sub2(n3, in.hS), mul2(n1, -1.0f));
+        const F2 hi = sel2(c4, zero, min2(e, zero));
+        F2 w = sub2(hi, lo);
+#pragma unroll
+        for (int i = 0; i < 20; ++i) {
+            w = mul2(w, 0.5f);
+            const F2 mid = add2(lo, w);
+            const F2 F = fma2(fma2(mid, mid, np), mid, nr);
+            lo = sel2(gt2(F, zero), mid, lo);
+        }
+        const F2 d34 = max2(add2(sel2(c4, in.hS, n12), fma2(w, 0.5f, lo)), n2);  // floor; drops NaN
+        d = sel2(gt2(t1, mul2(n2, sub2(n2, n1))), d34, d);
+        return sel2(le2(n12, W), mul2(add2(W, n12), 0.5f), d);                  // (5)
+    }
+};
+
+// One pair through frame and method: eq. (2)-(5) -> method -> eq. (8).
+template <int METHOD>
+__device__ __forceinline__ F2 solve_pair_fast(F2 V0, F2 nx, F2 ny, F2 nz) {
+    const PairIn in = pair_reduce(V0, nx, ny, nz);
+    return pair_restore(V0, in.hS, PairSolver<METHOD>::reduced_offset(in));
+}
+
+// ---------------------------------------------------------------------------------------
+// forward map V0(d0, n) for two cells at once: eq. (2)-(4), (7), (11), (6)   (Listing 1,
+// PAPER.md:71-92), branch-free.  All five cases are brought to one quotient
+//   V = top + num / den,   top = 1/2 for (4), (5) and 0 for (1)-(3),
+// with the stable numerators of volume_cell() (plic_methods.cuh), t = d - n12, s = d - S/2:
+//   (1) d^3                                   / (6 q n3)
+//   (2) 3 d (d - n1) + n1^2                   / (6 n2 n3)        [n1-free, caption of Listing 1]
+//   (3) 6 q (n12/2 + t) - t^3                 / (6 q n3)
+//   (4) s (3/2 u - 2 s^2)                     / (6 q n3)         [u = 4 q - (n3 - n12)^2]
+//   (5) -|d0|                                 / n3               [(d - n12/2)/n3 = 1/2 - |d0|/n3]
+// so one division serves every case.  It is a reciprocal (SFU) with one Newton correction of
+// the quotient, i.e. within 1-2 ulp of the IEEE quotient.  den is floored at 1e-37: a zero
+// normal then gives 1/2 - |d0| / 1e-37 -> 1/2 for d0 = 0 and 0 otherwise, as documented.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ F2 volume_pair(F2 d0, F2 nx, F2 ny, F2 nz) {
+    const F2 a = abs2(nx), b = abs2(ny), c = abs2(nz);
+    const F2 n1 = F2{min3(a.x, b.x, c.x), min3(a.y, b.y, c.y)};
+    const F2 n3 = F2{max3(a.x, b.x, c.x), max3(a.y, b.y, c.y)};
+    const F2 n2 = max2(min2(a, b), min2(max2(a, b), c));
     const F2 n12 = add2(n1, n2);
-    const F2 W = mul2(V2, n3);                                                  // 2 V n3
-    const F2 Wn2 = mul2(W, n2);
-    const F2 x = mul2(Wn2, 3.0f);                                               // 6 V n2 n3
-    const F2 s1 = mul2(n1, n1);
     const F2 hS = mul2(add2(n12, n3), 0.5f);
-    // (2) and (1)
-    const F2 d2 = fma2(n1, 0.5f, sqrt2(max2(fma2(s1, -1.0f / 12.0f, Wn2), 0.0f)));
-    const F2 d1 = ex2_2(mul2(lg2_2(mul2(x, n1)), 1.0f / 3.0f));
-    F2 d = sel2(lt2(x, s1), d1, d2);
-    // (3)/(4)
+    const F2 ad0 = abs2(d0);
+    const F2 d = F2{fmaxf(hS.x - ad0.x, 0.0f), fmaxf(hS.y - ad0.y, 0.0f)};        // eq. (7)
     const F2 q = mul2(n1, n2);
+    const F2 q6 = mul2(q, 6.0f);
+    // (1), (2)
+    const F2 num1 = mul2(mul2(d, d), d);
+    const F2 num2 = fma2(mul2(d, 3.0f), sub2(d, n1), mul2(n1, n1));
+    // (3): 6 q (n12/2 + t) - t^3 with nt = -t = n12 - d in [0, n1]
+    const F2 nt = sub2(n12, d);
+    const F2 num3 = fma2(fma2(n12, 0.5f, mul2(nt, -1.0f)), q6, mul2(mul2(nt, nt), nt));
+    // (4): s (3/2 u - 2 s^2), 3/2 u = 6 q - 3/2 e^2
+    const F2 s_ = sub2(d, hS);
     const F2 e = sub2(n3, n12);
-    const F2 z = sub2(n12, W);
-    const F2 ee = mul2(e, e);
-    const F2 h = fma2(fma2(q, -6.0f, ee), e, mul2(mul2(q, z), -3.0f));          // F3(e)
-    const B2 c4 = B2{e.x < 0.0f && h.x > 0.0f, e.y < 0.0f && h.y > 0.0f};
-    const F2 R = sel2(c4, fma2(q, 4.0f, mul2(ee, -1.0f)), mul2(q, 8.0f));
-    const F2 rho = rsqrt2(R);
-    const F2 K4 = mul2(mul2(mul2(q, 6.0f), sub2(n3, W)), mul2(rho, rho));
-    const F2 C = mul2(sel2(c4, K4, mul2(z, 1.5f)), rho);
-    const F2 ng = neg_sin_third_asin_fast2(C);
-    const F2 d34 = max2(fma2(mul2(R, rho), ng, sel2(c4, hS, n12)), n2);         // floor; drops NaN
-    d = sel2(gt2(x, fma2(mul2(n2, 3.0f), sub2(n2, n1), s1)), d34, d);
-    d = sel2(le2(n12, W), mul2(add2(W, n12), 0.5f), d);                         // (5)
-    d = min2(d, hS);
-    const F2 r = sub2(hS, d);
-    // eq. (8): the sign of V0 - 1/2 on r >= 0
-    const F2 t = fma2(V0, -1.0f, f2(0.5f));
-    return F2{__uint_as_float(__float_as_uint(r.x) | (~__float_as_uint(t.x) & 0x80000000u)),
-              __uint_as_float(__float_as_uint(r.y) | (~__float_as_uint(t.y) & 0x80000000u))};
+    const F2 u15 = fma2(mul2(e, e), -1.5f, q6);
+    const F2 num4 = mul2(s_, fma2(mul2(s_, s_), -2.0f, u15));
+    // case selection in the order of volume_cell(): (5), (1), (2), (3), else (4)
+    const B2 c5 = B2{d.x >= n12.x, d.y >= n12.y};
+    const B2 c1 = lt2(d, n1);
+    const B2 c2 = le2(d, n2);
+    const B2 c3 = le2(d, n3);
+    F2 num = sel2(c3, num3, num4);
+    num = sel2(c2, num2, num);
+    num = sel2(c1, num1, num);
+    num = sel2(c5, F2{-ad0.x, -ad0.y}, num);
+    const B2 use_n2 = andnot2(c2, c1);                                           // case (2)
+    F2 den = mul2(mul2(n3, 6.0f), sel2(use_n2, n2, q));
+    den = max2(sel2(c5, n3, den), 1e-37f);
+    const B2 top = B2{c5.x || !c3.x, c5.y || !c3.y};                             // (4) or (5)
+    // V = top + num/den:  nr = -1/den,  nv = -num/den,  corrected by err = num - den (num/den)
+    const F2 nr = F2{mufu_rcp(-den.x), mufu_rcp(-den.y)};
+    const F2 nv = mul2(num, nr);
+    const F2 nv2 = fma2(fma2(den, nv, num), nr, nv);
+    F2 V = fma2(nv2, -1.0f, sel2(top, f2(0.5f), f2(0.0f)));
+    V = min2(max2(V, 0.0f), f2(0.5f));
+    const F2 Vc = fma2(V, -1.0f, f2(1.0f));
+    return sel2(gt2(d0, f2(0.0f)), Vc, V);                                       // eq. (6)
 }
 
 }  // namespace plic
