@@ -15,7 +15,9 @@ shape with the sizes BASELINE.json's ``configs`` name; the recipe is restated
 in DESIGN.md.
 """
 from .workloads import (CHUNK, random_sphere, edge_cells, config1, snapped_beta,
-                        paper_benchmark_set, sphere_lattice, shard_range)
+                        paper_benchmark_set, paper_normals, roundtrip_volumes, sphere_lattice,
+                        shard_range)
 
 __all__ = ["CHUNK", "random_sphere", "edge_cells", "config1", "snapped_beta",
-           "paper_benchmark_set", "sphere_lattice", "shard_range"]
+           "paper_benchmark_set", "paper_normals", "roundtrip_volumes", "sphere_lattice",
+           "shard_range"]

@@ -20,6 +20,7 @@ _STREAM_SPHERE = 1
 _STREAM_EDGE = 2
 _STREAM_SNAP = 3
 _STREAM_PAPER = 4
+_STREAM_PAPER_NORMALS = 5
 
 _INV_SQRT2_F32 = np.float32(0.70710677)
 
@@ -166,6 +167,37 @@ def paper_benchmark_set(n_normals: int, L: int, seed: int):
     V0 = np.tile(v, n_normals)
     nx, ny, nz = (np.repeat(n[:, i], L) for i in range(3))
     return V0, nx, ny, nz
+
+
+def roundtrip_volumes(L: int):
+    """The L volumes plic_roundtrip_error steps through (include/plic.h): fp32 l*h with
+    h = fp32(1/(L-1)), the last one exactly 1 (the paper's "equally spaced, edge cases
+    included", PAPER.md:250)."""
+    h = np.float32(1.0) / np.float32(L - 1)
+    v = np.arange(L, dtype=np.float32) * h
+    v[L - 1] = np.float32(1.0)
+    return v.astype(np.float32)
+
+
+def paper_normals(n_normals: int, seed: int, workers=None):
+    """The normal set of the paper's GPU test at any size: normal 0 is
+    (1,0,0), normal 1 is (1/sqrt2, 1/sqrt2, 0), normals 2 .. n_normals/8 - 1 are random 2D
+    directions in the x-y plane, the rest random 3D directions (67108864 normals in the
+    paper: 8388606 2D, 58720256 3D).  Chunked like random_sphere.  Returns nx, ny, nz."""
+    n2d = max(n_normals // 8, 2)
+
+    def fn(c):
+        g = _rng(seed, _STREAM_PAPER_NORMALS, c).standard_normal((CHUNK, 3))
+        idx = c * CHUNK + np.arange(CHUNK)
+        g[idx < n2d, 2] = 0.0
+        n = _unit_rows(g)
+        if c == 0:
+            n[0] = (1.0, 0.0, 0.0)
+            n[1] = (np.sqrt(0.5), np.sqrt(0.5), 0.0)
+        return np.zeros(CHUNK, dtype=np.float32), n.astype(np.float32)
+
+    _, nx, ny, nz = _run_chunks(fn, 0, n_normals, workers)
+    return nx, ny, nz
 
 
 def sphere_lattice(L: int = 256, R: float = 60.0, centre=(128.3, 127.7, 128.1), sub: int = 8):

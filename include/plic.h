@@ -41,6 +41,8 @@ typedef struct CUstream_st *cudaStream_t;
 #define PLIC_METHOD_NESTED   3 /* nested intervals (bisection) for cases (3),(4): sect. 2.5,
                                   Listing 5 */
 #define PLIC_NUM_METHODS     4
+#define PLIC_METHOD_BLANK 0x40 /* plic_roundtrip_error only: the "blank run" of eq. (33), d0 = V0 - 1/2
+                                  in place of a PLIC solve */
 #define PLIC_FAST        0x100 /* approximate SFU roots/reciprocals/trig and branch-free,
                                   a-priori case selection; without it: IEEE division and
                                   square root, CUDA libm cbrt/asin/acos/sin/cos */
@@ -91,6 +93,31 @@ int plic_volume(const float *d0, const float *nx, const float *ny, const float *
                 float *V0, int64_t N, cudaStream_t stream);
 
 /*
+ * plic_roundtrip_error -- the paper's accuracy and timing benchmark (sect. 2.6):
+ * for each of N normals, the volume is varied over [0,1] in L equally spaced steps IN SERIES
+ * inside one thread, and
+ *
+ *     E[i] = (1/L) sum_l | plic_volume(plic_solve(V0_l, n_i), n_i) - V0_l |      (eq. (31))
+ *
+ * is stored, so that E_avg of eq. (32) is the mean of E over i.  With method =
+ * PLIC_METHOD_BLANK the solve is replaced by d0 = V0_l - 1/2 (eq. (33)); the paper's time per
+ * PLIC evaluation is (t(method) - t(blank)) / (N L).  The loop reads 12 B and writes 4 B per
+ * normal for L evaluations, so unlike plic_solve this entry point is compute bound.
+ * The volumes are generated in the kernel: V0_l = fl(l * h) for l = 0..L-2 with
+ * h = fl(1 / (L-1)) (fp32 multiplication and division), and V0_{L-1} = 1 exactly
+ * (gen.roundtrip_volumes(L) returns the same values).  The sum runs in fp32 over even l and
+ * over odd l separately, in increasing l, and the two partial sums are then added.
+ *
+ *   nx, ny, nz   DEVICE pointers, fp32, N elements each, read only.
+ *   E            DEVICE pointer, fp32, N elements, written.
+ *   N >= 0, L >= 2;  method = PLIC_METHOD_* [| PLIC_FAST] or PLIC_METHOD_BLANK.
+ *
+ * Errors, ownership and stream semantics as plic_solve (PLIC_ERR_SIZE also for L < 2).
+ */
+int plic_roundtrip_error(const float *nx, const float *ny, const float *nz, float *E, int64_t N,
+                         int L, int method, cudaStream_t stream);
+
+/*
  * plic_solve_host / plic_volume_host -- the same maps for HOST arrays (pageable or pinned;
  * pinned memory makes the copies asynchronous).  The range is cut into chunks; host->device
  * copies, the kernel and the device->host copy of consecutive chunks overlap on three
@@ -106,7 +133,7 @@ int plic_volume_host(const float *d0, const float *nx, const float *ny, const fl
 /* Frees the host-API workspace and streams of every device; safe to call at any time. */
 void plic_host_release(void);
 
-/* "analytic", "sz", "newton", "nested" (+ "-fast" with PLIC_FAST); NULL if unknown.
+/* "analytic", "sz", "newton", "nested" (+ "-fast" with PLIC_FAST), "blank"; NULL if unknown.
  * The string is static storage owned by the library. */
 const char *plic_method_name(int method);
 

@@ -10,6 +10,8 @@ shared library is missing it is built with nvcc, and if that fails the import ra
     plic_solve(V0, nx, ny, nz, out=None, method="analytic", fast=False, stream=None) -> d0
     plic_volume(d0, nx, ny, nz, out=None, stream=None) -> V0
     plic_solve_host / plic_volume_host      same maps for host arrays (numpy or CPU tensors)
+    plic_roundtrip_error(nx, ny, nz, L, out=None, method="analytic", fast=False) -> E
+                                            the paper's benchmark loop, eq. (31)-(33)
 """
 from __future__ import annotations
 
@@ -18,13 +20,15 @@ import os
 
 from . import build as _build
 
-__all__ = ["METHODS", "FAST", "method_id", "plic_solve", "plic_volume", "plic_solve_host",
+__all__ = ["METHODS", "FAST", "BLANK", "method_id", "plic_solve", "plic_volume",
+           "plic_roundtrip_error", "plic_solve_host",
            "plic_volume_host", "plic_host_release", "plic_method_name", "plic_error_string",
            "plic_version", "plic_launch_config", "plic_launch_count", "PlicError", "lib",
            "LIB_PATH"]
 
 METHODS = {"analytic": 0, "sz": 1, "newton": 2, "nested": 3}
 FAST = 0x100
+BLANK = 0x40            # plic_roundtrip_error only: the blank run of eq. (33)
 LIB_PATH = _build.LIB
 
 
@@ -44,6 +48,9 @@ def _load() -> ctypes.CDLL:
     lib_.plic_solve.restype = ctypes.c_int
     lib_.plic_volume.argtypes = [fp, fp, fp, fp, fp, i64, ctypes.c_void_p]
     lib_.plic_volume.restype = ctypes.c_int
+    lib_.plic_roundtrip_error.argtypes = [fp, fp, fp, fp, i64, ctypes.c_int, ctypes.c_int,
+                                          ctypes.c_void_p]
+    lib_.plic_roundtrip_error.restype = ctypes.c_int
     lib_.plic_solve_host.argtypes = [fp, fp, fp, fp, fp, i64, ctypes.c_int]
     lib_.plic_solve_host.restype = ctypes.c_int
     lib_.plic_volume_host.argtypes = [fp, fp, fp, fp, fp, i64]
@@ -72,6 +79,8 @@ def method_id(method, fast: bool = False) -> int:
         name = method
         if name.endswith("-fast"):
             name, fast = name[:-5], True
+        if name == "blank":
+            return BLANK
         if name not in METHODS:
             raise ValueError("unknown PLIC method %r" % (method,))
         mid = METHODS[name]
@@ -159,6 +168,21 @@ def plic_volume(d0, nx, ny, nz, out=None, stream=None):
                              out.data_ptr(), N, _stream_handle(stream, d0.device))
     if rc != 0:
         raise PlicError(rc, "plic_volume")
+    return out
+
+
+def plic_roundtrip_error(nx, ny, nz, L: int, out=None, method="analytic", fast: bool = False,
+                         stream=None):
+    """E[i] = mean over L equally spaced V0 of |plic_volume(plic_solve(V0, n_i), n_i) - V0|
+    (eq. (31), PAPER.md:233); method "blank" = eq. (33).  Returns `out`."""
+    import torch
+    N, out = _device_args(nx, nx, ny, nz, out)
+    with torch.cuda.device(nx.device):
+        rc = lib.plic_roundtrip_error(nx.data_ptr(), ny.data_ptr(), nz.data_ptr(), out.data_ptr(),
+                                      N, int(L), method_id(method, fast),
+                                      _stream_handle(stream, nx.device))
+    if rc != 0:
+        raise PlicError(rc, "plic_roundtrip_error")
     return out
 
 

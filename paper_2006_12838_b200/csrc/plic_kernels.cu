@@ -355,6 +355,70 @@ static int launch_map(int k, const float *s, const float *nx, const float *ny, c
 }
 
 // ---------------------------------------------------------------------------------------
+// roundtrip_kernel: the paper's benchmark loop (sect. 2.6, eq. (31)-(33)).  One thread per
+// normal; L volumes in series, two per step on a packed pair (V0_l, V0_{l+1}) that shares
+// the normal, so everything that depends on n alone is hoisted out of the loop by the
+// compiler -- the same situation as the paper's OpenCL kernel.
+// METHOD = -1 is the blank run of eq. (33).
+// ---------------------------------------------------------------------------------------
+template <int METHOD, bool FAST>
+struct PairOffset {                                   // precise kernels: two scalar solves
+    static __device__ __forceinline__ F2 d0(F2 V0, F2 x, F2 y, F2 z) {
+        return F2{solve_cell<METHOD, false>(V0.x, x.x, y.x, z.x),
+                  solve_cell<METHOD, false>(V0.y, x.y, y.y, z.y)};
+    }
+};
+template <int METHOD>
+struct PairOffset<METHOD, true> {
+    static __device__ __forceinline__ F2 d0(F2 V0, F2 x, F2 y, F2 z) {
+        return solve_pair_fast<METHOD>(V0, x, y, z);
+    }
+};
+template <>
+struct PairOffset<-1, true> {
+    static __device__ __forceinline__ F2 d0(F2 V0, F2, F2, F2) { return add2(V0, f2(-0.5f)); }
+};
+
+template <int METHOD, bool FAST>
+__global__ void __launch_bounds__(kBlock)
+roundtrip_kernel(const float *__restrict__ nx, const float *__restrict__ ny,
+                 const float *__restrict__ nz, float *__restrict__ E, int64_t N, int L) {
+    const float h = 1.0f / (float)(L - 1);
+    const int64_t stride = (int64_t)gridDim.x * kBlock;
+    for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < N; i += stride) {
+        const float x = nx[i], y = ny[i], z = nz[i];
+        const F2 X{x, x}, Y{y, y}, Z{z, z};
+        F2 acc{0.0f, 0.0f};
+        for (int l = 0; l < L; l += 2) {
+            // V0_l = l / (L - 1); the last one is exactly 1.  For odd L the second half of the
+            // last pair is a repeat of V0 = 1 and is not accumulated.
+            const F2 V0{l >= L - 1 ? 1.0f : (float)l * h, l + 1 >= L - 1 ? 1.0f : (float)(l + 1) * h};
+            const F2 V = volume_pair(PairOffset<METHOD, FAST>::d0(V0, X, Y, Z), X, Y, Z);
+            const F2 err = abs2(sub2(V, V0));                                   // eq. (31)
+            acc.x += err.x;
+            if (l + 1 < L) acc.y += err.y;
+        }
+        E[i] = (acc.x + acc.y) / (float)L;
+    }
+}
+
+typedef void (*roundtrip_kernel_t)(const float *, const float *, const float *, float *, int64_t,
+                                   int);
+static roundtrip_kernel_t roundtrip_kernel_of(int k) {
+    switch (k) {
+        case 0: return roundtrip_kernel<ANALYTIC, false>;
+        case 1: return roundtrip_kernel<SZ, false>;
+        case 2: return roundtrip_kernel<NEWTON, false>;
+        case 3: return roundtrip_kernel<NESTED, false>;
+        case 4: return roundtrip_kernel<ANALYTIC, true>;
+        case 5: return roundtrip_kernel<SZ, true>;
+        case 6: return roundtrip_kernel<NEWTON, true>;
+        case 7: return roundtrip_kernel<NESTED, true>;
+        default: return roundtrip_kernel<-1, true>;
+    }
+}
+
+// ---------------------------------------------------------------------------------------
 // host-array API: chunked, three-stage pipeline (H2D | kernel | D2H) over three streams
 // ---------------------------------------------------------------------------------------
 constexpr int kSlots = 3;
@@ -445,6 +509,26 @@ int plic_volume(const float *d0, const float *nx, const float *ny, const float *
     return plic::launch_map(plic::kVolumeKernel, d0, nx, ny, nz, V0, N, stream);
 }
 
+int plic_roundtrip_error(const float *nx, const float *ny, const float *nz, float *E, int64_t N,
+                         int L, int method, cudaStream_t stream) {
+    const int k = method == PLIC_METHOD_BLANK ? plic::kVolumeKernel : plic::kernel_index(method);
+    if (k < 0) return PLIC_ERR_METHOD;
+    if (N < 0 || L < 2) return PLIC_ERR_SIZE;
+    if (N == 0) return PLIC_OK;
+    if (!nx || !ny || !nz || !E) return PLIC_ERR_NULL;
+    if (((uintptr_t)nx | (uintptr_t)ny | (uintptr_t)nz | (uintptr_t)E) & 3u) return PLIC_ERR_ALIGN;
+    cudaError_t err;
+    const plic::DeviceInfo *info = plic::device_info(&err);
+    if (!info) return PLIC_ERR_LAUNCH;
+    // compute bound: one thread per normal, at most 8 resident blocks per SM
+    const int64_t need = (N + plic::kBlock - 1) / plic::kBlock;
+    const int64_t full = (int64_t)info->sms * 8;
+    plic::roundtrip_kernel_of(k)<<<(int)(need < full ? need : full), plic::kBlock, 0, stream>>>(
+        nx, ny, nz, E, N, L);
+    plic::g_launches.fetch_add(1, std::memory_order_relaxed);
+    return cudaGetLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
+}
+
 int plic_solve_host(const float *V0, const float *nx, const float *ny, const float *nz,
                     float *d0, int64_t N, int method) {
     const int k = plic::kernel_index(method);
@@ -473,6 +557,7 @@ const char *plic_method_name(int method) {
     static const char *names[2 * PLIC_NUM_METHODS] = {
         "analytic",      "sz",      "newton",      "nested",
         "analytic-fast", "sz-fast", "newton-fast", "nested-fast"};
+    if (method == PLIC_METHOD_BLANK) return "blank";
     const int k = plic::kernel_index(method);
     return k < 0 ? nullptr : names[k];
 }

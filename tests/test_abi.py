@@ -25,7 +25,7 @@ def _declared_functions():
 
 def test_header_declares_the_boundary():
     names = _declared_functions()
-    for must in ("plic_solve", "plic_volume", "plic_solve_host", "plic_volume_host",
+    for must in ("plic_solve", "plic_volume", "plic_roundtrip_error", "plic_solve_host", "plic_volume_host",
                  "plic_method_name", "plic_version", "plic_launch_count"):
         assert must in names
 
@@ -50,6 +50,7 @@ def test_version_and_names(plic):
     assert [plic.plic_method_name(i) for i in range(4)] == ["analytic", "sz", "newton", "nested"]
     assert plic.plic_method_name(2 | plic.FAST) == "newton-fast"
     assert plic.plic_method_name(4) is None and plic.plic_method_name(-1) is None
+    assert plic.plic_method_name(plic.BLANK) == "blank"
     assert plic.plic_error_string(0) == "ok"
     for code in (-1, -2, -3, -4, -5):
         assert plic.plic_error_string(code) not in ("ok", "unknown error code")
@@ -60,6 +61,7 @@ def test_method_id_marshalling(plic):
     assert plic.method_id("sz", fast=True) == 0x101
     assert plic.method_id("nested-fast") == 0x103
     assert plic.method_id(2) == 2
+    assert plic.method_id("blank") == 0x40
     with pytest.raises(ValueError):
         plic.method_id("kawano")
 
@@ -82,6 +84,13 @@ def test_argument_validation_needs_no_device(plic):
     assert lib.plic_solve(p, p, p, p, p, 4, 7, None) == -3
     assert lib.plic_solve(p, p, p, p, p, 4, 0x204, None) == -3
     assert lib.plic_solve_host(p, p, p, p, p, 4, -1) == -3
+    # plic_roundtrip_error: sizes, method (blank allowed here, not in plic_solve), null
+    assert lib.plic_roundtrip_error(None, None, None, None, 0, 256, 0, None) == 0
+    assert lib.plic_roundtrip_error(p, p, p, p, 4, 1, 0, None) == -2
+    assert lib.plic_roundtrip_error(p, p, p, p, -4, 256, 0, None) == -2
+    assert lib.plic_roundtrip_error(p, p, p, p, 4, 256, 9, None) == -3
+    assert lib.plic_roundtrip_error(p, p, None, p, 4, 256, 0x40, None) == -1
+    assert lib.plic_solve(p, p, p, p, p, 4, 0x40, None) == -3
     # misaligned (not a multiple of 4 bytes)
     q = ctypes.c_void_p(p.value + 2)
     assert lib.plic_solve(q, p, p, p, p, 1, 0, None) == -5

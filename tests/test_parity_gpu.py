@@ -344,3 +344,66 @@ def test_sphere_lattice(plic):
         n_ref = int((dev_ref > 0.05).sum())
         assert n_ref <= 8
         assert (dev_gpu > 0.05 + 4e-5).sum() <= n_ref <= (dev_gpu > 0.05 - 4e-5).sum()
+
+
+# ------------------------------------------------------------------------------------------
+# plic_roundtrip_error: the paper's benchmark loop (sect. 2.6, eq. (31)-(33))
+# ------------------------------------------------------------------------------------------
+RT_VARIANTS = VARIANTS + [("blank", False)]
+RT_IDS = IDS + ["blank"]
+
+
+def _composed_roundtrip(plic, nx, ny, nz, L, method, fast):
+    """eq. (31) assembled from the two parity-tested entry points, with the summation order
+    include/plic.h states (fp32; even l and odd l separately, then added)."""
+    n = len(nx)
+    v = gen.roundtrip_volumes(L)
+    V0 = np.tile(v, n)
+    ax, ay, az = (np.repeat(a, L) for a in (nx, ny, nz))
+    tV, tx, ty, tz = dev(V0, ax, ay, az)
+    if method == "blank":
+        d0 = tV - 0.5                                                   # eq. (33), exact in fp32
+    else:
+        d0 = plic.plic_solve(tV, tx, ty, tz, method=method, fast=fast)
+    V = plic.plic_volume(d0, tx, ty, tz)
+    err = (V - tV).abs().cpu().numpy().reshape(n, L)
+    acc = np.zeros((n, 2), dtype=np.float32)
+    for l in range(L):
+        acc[:, l & 1] += err[:, l]
+    return (acc[:, 0] + acc[:, 1]) / np.float32(L), d0.cpu().numpy().reshape(n, L)
+
+
+@pytest.mark.parametrize("L", [256, 17, 2])
+@pytest.mark.parametrize("method,fast", RT_VARIANTS, ids=RT_IDS)
+def test_roundtrip_error_kernel(plic, method, fast, L):
+    n = 3001
+    nx, ny, nz = gen.paper_normals(n, seed=21)         # (1,0,0), face diagonal, 2-D, 3-D normals
+    tx, ty, tz = dev(nx, ny, nz)
+    before = plic.plic_launch_count()
+    E = plic.plic_roundtrip_error(tx, ty, tz, L, method=method, fast=fast).cpu().numpy()
+    assert plic.plic_launch_count() == before + 1
+    assert E.shape == (n,) and np.all(np.isfinite(E))                   # no NaN at n = (1,0,0), V0 in {0,1}
+    # (a) the fused loop equals the composition of plic_solve and plic_volume (both held to the
+    #     oracle above); the few-ulp slack covers fused-multiply-add contraction differences
+    E_comp, d0 = _composed_roundtrip(plic, nx, ny, nz, L, method, fast)
+    assert np.max(np.abs(E - E_comp)) <= 2e-8, np.max(np.abs(E - E_comp))
+    # (b) against the oracle: the fp64 round trip is exact (pinned to 1e-12), so E is the
+    #     method's forward-volume residual, bounded as in north_star
+    v = gen.roundtrip_volumes(L).astype(np.float64)
+    if method == "blank":
+        ax, ay, az = (np.repeat(a, L) for a in (nx, ny, nz))
+        ref = np.abs(oracle.volume((np.tile(v, n) - 0.5).astype(np.float32), ax, ay, az) - np.tile(v, n))
+        E_ref = ref.reshape(n, L).mean(axis=1)
+        assert np.max(np.abs(E - E_ref)) <= TOL_VOL
+    else:
+        assert E.max() <= TOL_RES
+        # fp32 error scale of Tables 1 and 3 (2e-8 .. 7e-8): same order here
+        assert E.astype(np.float64).mean() <= 3e-7, E.mean()
+
+
+def test_roundtrip_error_empty_and_validation(plic):
+    tx = torch.zeros(0, device="cuda")
+    assert plic.plic_roundtrip_error(tx, tx, tx, 8).shape == (0,)
+    t = torch.ones(4, device="cuda")
+    with pytest.raises(plic.PlicError):
+        plic.plic_roundtrip_error(t, t, t, 1)
