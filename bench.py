@@ -18,6 +18,11 @@ Multi-GPU (torchrun, one rank per GPU): the path has no exchange step, so rank r
 own 2^26 cells [r 2^26, (r+1) 2^26) of the same seeded stream, no data-path collective;
 `value` = all ranks' cells / max-over-ranks time ("scaling": "weak").
 
+"paper_benchmark" is the paper's own benchmark shape (sect. 2.6, Table 3) through
+plic_roundtrip_error: 2^k normals x L = 256 volumes in series per thread, blank run (eq. 33)
+subtracted, ps per PLIC evaluation and E_avg (eq. 32) per method -- compute bound, for
+comparison with the paper's Titan Xp column (context, not the target).
+
 --impl reference times the fp64 CPU oracle (oracle/), as it stands, on the host cores.
 """
 from __future__ import annotations
@@ -304,6 +309,7 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
 
     variants = [(m, f) for f in (True, False) for m in ("analytic", "sz", "newton", "nested")]
+    solve_names_all = [m + ("-fast" if f else "") for m, f in variants]
     sampler = ClockSampler(local)
     sampler.start()
 
@@ -339,6 +345,27 @@ def run_ours(args):
                               "hbm_gbs_per_gpu": BYTES_PER_CELL * N * args.steps / (ms * 1e-3) / 1e9}
     windows["plic_volume"] = win
     total_launches = plic.plic_launch_count() - launches_before
+
+    # ---- the paper's own benchmark shape (sect. 2.6, Table 3): compute bound, blank run subtracted
+    paper = None
+    if args.paper_log2n > 0:
+        PN, PL = 1 << args.paper_log2n, 256
+        pn = [torch.from_numpy(a).cuda() for a in gen.paper_normals(PN, 5)]
+        pE = torch.empty_like(pn[0])
+        paper = {"normals": PN, "L": PL, "unit": "ps per PLIC evaluation, blank run (eq. 33) subtracted",
+                 "paper_titan_xp_ps": {"sz": 12.8, "analytic": 19.0, "newton": 19.2, "nested": 106.4},
+                 "methods": {}}
+        pnames = ["blank"] + solve_names_all
+        raw = {}
+        for name in pnames:
+            ms, _ = time_launches(lambda: plic.plic_roundtrip_error(*pn, PL, out=pE, method=name),
+                                  3, 3, stream)
+            raw[name] = (max_over_ranks(ms) / 3, float(pE.double().mean()))
+        for name in pnames:
+            ms, eavg = raw[name]
+            paper["methods"][name] = {"ms": ms, "ps_per_eval": (ms - raw["blank"][0]) * 1e9 / (PN * PL),
+                                      "ps_per_eval_incl_blank": ms * 1e9 / (PN * PL), "E_avg": eavg}
+        del pn, pE
 
     solve_names = [plic.plic_method_name(plic.method_id(m, f)) for m, f in variants]
     head = args.method if args.method != "auto" else max(solve_names, key=lambda k: methods[k]["value"])
@@ -397,6 +424,8 @@ def run_ours(args):
                          "algorithmic_bytes_per_launch": BYTES_PER_CELL * N, "peak_source": peak_src},
             "methods": methods,
         }
+        if paper is not None:
+            line["paper_benchmark"] = paper
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(host)
         print(json.dumps(line), flush=True)
@@ -418,6 +447,9 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--prewarm-ms", type=float, default=300.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--paper-log2n", type=int, default=24,
+                    help="normals in the paper-shaped compute-bound leg = 2^k, L = 256 volumes each "
+                         "(the paper: k = 26); 0 skips it")
     args = ap.parse_args(argv)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                       # timing rule: at least 3 warm-up steps

@@ -267,44 +267,4 @@ __device__ __forceinline__ float solve_cell(float V0, float nx, float ny, float 
     return V0 > 0.5f ? r : -r;                                         // eq. (8)
 }
 
-// ---------------------------------------------------------------------------------------
-// forward map V0(d0, n): eq. (2)-(4), (7), (11), (6)   (Listing 1)
-//
-// Case (5) first and case (2) in its n1-free form, so n1 = 0 and n1 = n2 = 0 never divide
-// by zero (caption of Listing 1).  Cases (3) and (4) are evaluated in the expanded forms
-//   (3): V = (n12/2 + t - t^3/(6 n1 n2)) / n3,                 t = d - n12 in [-n1, 0]
-//   (4): V = 1/2 + s (3 u/4 - s^2) / (3 n1 n2 n3),             s = d - S/2 in [-n1/2, 0]
-// instead of the fdim-merged difference of cubes of Listing 1: that difference cancels to
-// ~eps d^3/(6 n1 n2 n3) in fp32, i.e. 4e-3 for n1 = 1e-6 ("forward map").
-// ---------------------------------------------------------------------------------------
-__device__ __forceinline__ float volume_cell(float d0, float nx, float ny, float nz) {
-    const float a = fabsf(nx), b = fabsf(ny), c = fabsf(nz);
-    const float n1 = min3(a, b, c);
-    const float n3 = max3(a, b, c);
-    const float n2 = fmaxf(fminf(a, b), fminf(fmaxf(a, b), c));
-    const float n12 = n1 + n2;
-    const float hS = 0.5f * (n12 + n3);
-    const float d = fmaxf(hS - fabsf(d0), 0.0f);                        // eq. (7)
-    float V;
-    if (n3 == 0.0f) {
-        V = d0 == 0.0f ? 0.5f : 0.0f;                                   // zero normal
-    } else if (d >= n12) {
-        V = (d - 0.5f * n12) / n3;                                      // (5)
-    } else if (d < n1) {
-        V = (d * d) / (6.0f * n2 * n3) * (d / n1);                      // (1)
-    } else if (d <= n2) {
-        V = fmaf(3.0f * d, d - n1, n1 * n1) / (6.0f * n2 * n3);         // (2)
-    } else if (d <= n3) {
-        const float t = d - n12;                                        // (3)
-        V = (fmaf(0.5f, n12, t) - (t * t) / (6.0f * n2) * (t / n1)) / n3;
-    } else {
-        const float e = n3 - n12;                                       // (4)
-        const float u = fmaf(4.0f, n1 * n2, -e * e);
-        const float s = d - hS;
-        V = fmaf(fmaf(0.75f, u, -s * s) / (3.0f * n2 * n3), s / n1, 0.5f);
-    }
-    V = fminf(fmaxf(V, 0.0f), 0.5f);
-    return d0 > 0.0f ? 1.0f - V : V;                                    // eq. (6)
-}
-
 }  // namespace plic

@@ -330,13 +330,19 @@ __device__ __forceinline__ F2 solve_pair_fast(F2 V0, F2 nx, F2 ny, F2 nz) {
 
 // ---------------------------------------------------------------------------------------
 // forward map V0(d0, n) for two cells at once: eq. (2)-(4), (7), (11), (6)   (Listing 1,
-// PAPER.md:71-92), branch-free.  All five cases are brought to one quotient
-//   V = top + num / den,   top = 1/2 for (4), (5) and 0 for (1)-(3),
-// with the stable numerators of volume_cell() (plic_methods.cuh), t = d - n12, s = d - S/2:
+// PAPER.md:71-92), branch-free.  Case (5) is tested first and case (2) is in its n1-free form,
+// so n1 = 0 and n1 = n2 = 0 never divide by zero (caption of Listing 1).  Cases (3) and (4) are
+// evaluated in forms expanded around d = n12 resp. d = S/2,
+//   (3): V = (n12/2 + t - t^3/(6 q)) / n3,          t = d - n12 in [-n1, 0]
+//   (4): V = 1/2 + s (3 u/4 - s^2) / (3 q n3),      s = d - S/2 in [-n1/2, 0],  u = 4 q - (n3 - n12)^2
+// instead of the fdim-merged difference of cubes of Listing 1: that difference cancels to
+// ~eps d^3/(6 n1 n2 n3) in fp32, i.e. 4e-3 for n1 = 1e-6 ("forward map").
+// All five cases are brought to one quotient
+//   V = top + num / den,   top = 1/2 for (4), (5) and 0 for (1)-(3):
 //   (1) d^3                                   / (6 q n3)
-//   (2) 3 d (d - n1) + n1^2                   / (6 n2 n3)        [n1-free, caption of Listing 1]
+//   (2) 3 d (d - n1) + n1^2                   / (6 n2 n3)
 //   (3) 6 q (n12/2 + t) - t^3                 / (6 q n3)
-//   (4) s (3/2 u - 2 s^2)                     / (6 q n3)         [u = 4 q - (n3 - n12)^2]
+//   (4) s (3/2 u - 2 s^2)                     / (6 q n3)
 //   (5) -|d0|                                 / n3               [(d - n12/2)/n3 = 1/2 - |d0|/n3]
 // so one division serves every case.  It is a reciprocal (SFU) with one Newton correction of
 // the quotient, i.e. within 1-2 ulp of the IEEE quotient.  den is floored at 1e-37: a zero
@@ -364,7 +370,7 @@ __device__ __forceinline__ F2 volume_pair(F2 d0, F2 nx, F2 ny, F2 nz) {
     const F2 e = sub2(n3, n12);
     const F2 u15 = fma2(mul2(e, e), -1.5f, q6);
     const F2 num4 = mul2(s_, fma2(mul2(s_, s_), -2.0f, u15));
-    // case selection in the order of volume_cell(): (5), (1), (2), (3), else (4)
+    // case selection: (5) first, then (1), (2), (3), else (4)
     const B2 c5 = B2{d.x >= n12.x, d.y >= n12.y};
     const B2 c1 = lt2(d, n1);
     const B2 c2 = le2(d, n2);
