@@ -187,14 +187,20 @@ def oracle_rate(arrays, n_cells: int):
 
 
 def cpu_baseline(arrays, budget_s: float = 12.0):
+    """The oracle as it stands on all host threads, for about budget_s seconds: a prefix of the
+    workload sized from a calibration pass, repeated when the whole workload takes less."""
     import oracle
     N = arrays[0].shape[0]
     cal = min(N, 1 << 20)
     rate, _ = oracle_rate(arrays, cal)                       # calibration (also warms the .so)
     n = int(min(N, max(cal, rate * budget_s)))
-    rate, dt = oracle_rate(arrays, n)
-    return {"value": rate / 1e9, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
-            "sample": "first %d cells of the workload (%.1f s of fp64 bisection, all host threads)" % (n, dt)}
+    passes, cells, secs = 0, 0, 0.0
+    while passes == 0 or (secs < 0.8 * budget_s and passes < 64):
+        _, dt = oracle_rate(arrays, n)
+        passes, cells, secs = passes + 1, cells + n, secs + dt
+    return {"value": cells / secs / 1e9, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+            "sample": "first %d cells of the workload x %d passes (%.1f s of fp64 bisection, all host "
+                      "threads)" % (n, passes, secs)}
 
 
 def run_reference(args):
