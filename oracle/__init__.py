@@ -10,6 +10,9 @@ lives entirely in the C file, whose header cites the paper passages it follows
     volume(d0, nx, ny, nz) -> V0      forward map, eq. (11)+(6)+(7)
     solve(V0, nx, ny, nz)  -> d0      bisection of the forward map on [-S/2, S/2]
     case(d0, nx, ny, nz)   -> 1..5    intersection case of eq. (11)
+
+Sub-modules (numpy fp64, same rules): ``oracle.sphere`` -- the plane-sphere problem of sect. 3
+(eq. (37) and its inverse by bisection).
 """
 from __future__ import annotations
 
