@@ -350,6 +350,18 @@ def run_ours(args):
                               "ms_per_step": ms / args.steps, "launches": args.steps,
                               "hbm_gbs_per_gpu": BYTES_PER_CELL * N * args.steps / (ms * 1e-3) / 1e9}
     windows["plic_volume"] = win
+    # plane-sphere maps of sect. 3: one array in, one out (8 B per cell)
+    sphere_names = []
+    for name, fn in (("sphere_solve-fast", lambda: plic.plic_sphere_solve(dV, out=out, fast=True)),
+                     ("sphere_solve", lambda: plic.plic_sphere_solve(dV, out=out, fast=False)),
+                     ("sphere_volume", lambda: plic.plic_sphere_volume(out, out=vol))):
+        ms, win = time_launches(fn, args.steps, args.warmup, stream)
+        ms = max_over_ranks(ms)
+        methods[name] = {"value": N * world * args.steps / (ms * 1e-3) / 1e9,
+                         "ms_per_step": ms / args.steps, "launches": args.steps, "bytes_per_cell": 8,
+                         "hbm_gbs_per_gpu": 8 * N * args.steps / (ms * 1e-3) / 1e9}
+        windows[name] = win
+        sphere_names.append(name)
     total_launches = plic.plic_launch_count() - launches_before
 
     # ---- the paper's own benchmark shape (sect. 2.6, Table 3): compute bound, blank run subtracted

@@ -118,6 +118,23 @@ int plic_roundtrip_error(const float *nx, const float *ny, const float *nz, floa
                          int L, int method, cudaStream_t stream);
 
 /*
+ * plic_sphere_solve / plic_sphere_volume -- the plane-sphere intersection of sect. 3
+ * (PAPER.md:294-321): a sphere of unit volume (radius r = (3/(4 pi))^(1/3), eq. (34)) cut by
+ * a plane at offset d0 in [-r, r] from its centre; the direction of the normal is irrelevant.
+ *
+ *   plic_sphere_volume   V0[i] = pi/3 (r + d0[i])^2 (2r - d0[i])                  (eq. (37))
+ *   plic_sphere_solve    d0[i] = the offset with that volume, eq. (38)           (eq. (36))
+ *
+ * DEVICE pointers, fp32, N elements each; the output may be the same pointer as the input.
+ * fast = 0: IEEE sqrt and CUDA libm asin/sin/cos; fast = PLIC_FAST: SFU square roots and the
+ * polynomial sin(asin(.)/3) of the cube kernels.  V0 < 0 acts as 0, V0 > 1 as 1; |d0| > r gives
+ * 0 or 1.  8 B of HBM traffic per cell.  Errors, alignment, ownership and stream semantics as
+ * plic_solve (PLIC_ERR_METHOD for any other value of fast).
+ */
+int plic_sphere_solve(const float *V0, float *d0, int64_t N, int fast, cudaStream_t stream);
+int plic_sphere_volume(const float *d0, float *V0, int64_t N, cudaStream_t stream);
+
+/*
  * plic_solve_host / plic_volume_host -- the same maps for HOST arrays (pageable or pinned;
  * pinned memory makes the copies asynchronous).  The range is cut into chunks; host->device
  * copies, the kernel and the device->host copy of consecutive chunks overlap on three

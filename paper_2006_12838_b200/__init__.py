@@ -12,6 +12,8 @@ shared library is missing it is built with nvcc, and if that fails the import ra
     plic_solve_host / plic_volume_host      same maps for host arrays (numpy or CPU tensors)
     plic_roundtrip_error(nx, ny, nz, L, out=None, method="analytic", fast=False) -> E
                                             the paper's benchmark loop, eq. (31)-(33)
+    plic_sphere_solve(V0, out=None, fast=False) -> d0, plic_sphere_volume(d0, out=None) -> V0
+                                            the plane-sphere intersection of sect. 3
 """
 from __future__ import annotations
 
@@ -21,7 +23,7 @@ import os
 from . import build as _build
 
 __all__ = ["METHODS", "FAST", "BLANK", "method_id", "plic_solve", "plic_volume",
-           "plic_roundtrip_error", "plic_solve_host",
+           "plic_roundtrip_error", "plic_sphere_solve", "plic_sphere_volume", "plic_solve_host",
            "plic_volume_host", "plic_host_release", "plic_method_name", "plic_error_string",
            "plic_version", "plic_launch_config", "plic_launch_count", "PlicError", "lib",
            "LIB_PATH"]
@@ -51,6 +53,10 @@ def _load() -> ctypes.CDLL:
     lib_.plic_roundtrip_error.argtypes = [fp, fp, fp, fp, i64, ctypes.c_int, ctypes.c_int,
                                           ctypes.c_void_p]
     lib_.plic_roundtrip_error.restype = ctypes.c_int
+    lib_.plic_sphere_solve.argtypes = [fp, fp, i64, ctypes.c_int, ctypes.c_void_p]
+    lib_.plic_sphere_solve.restype = ctypes.c_int
+    lib_.plic_sphere_volume.argtypes = [fp, fp, i64, ctypes.c_void_p]
+    lib_.plic_sphere_volume.restype = ctypes.c_int
     lib_.plic_solve_host.argtypes = [fp, fp, fp, fp, fp, i64, ctypes.c_int]
     lib_.plic_solve_host.restype = ctypes.c_int
     lib_.plic_volume_host.argtypes = [fp, fp, fp, fp, fp, i64]
@@ -183,6 +189,30 @@ def plic_roundtrip_error(nx, ny, nz, L: int, out=None, method="analytic", fast: 
                                       _stream_handle(stream, nx.device))
     if rc != 0:
         raise PlicError(rc, "plic_roundtrip_error")
+    return out
+
+
+def plic_sphere_solve(V0, out=None, fast: bool = False, stream=None):
+    """d0 of the plane cutting the volume V0 off the unit-volume sphere (eq. (38)); returns `out`."""
+    import torch
+    N, out = _device_args(V0, V0, V0, V0, out)
+    with torch.cuda.device(V0.device):
+        rc = lib.plic_sphere_solve(V0.data_ptr(), out.data_ptr(), N, FAST if fast else 0,
+                                   _stream_handle(stream, V0.device))
+    if rc != 0:
+        raise PlicError(rc, "plic_sphere_solve")
+    return out
+
+
+def plic_sphere_volume(d0, out=None, stream=None):
+    """V0 cut off the unit-volume sphere by the plane at offset d0 (eq. (37)); returns `out`."""
+    import torch
+    N, out = _device_args(d0, d0, d0, d0, out)
+    with torch.cuda.device(d0.device):
+        rc = lib.plic_sphere_volume(d0.data_ptr(), out.data_ptr(), N,
+                                    _stream_handle(stream, d0.device))
+    if rc != 0:
+        raise PlicError(rc, "plic_sphere_volume")
     return out
 
 

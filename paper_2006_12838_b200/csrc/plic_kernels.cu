@@ -419,6 +419,76 @@ static roundtrip_kernel_t roundtrip_kernel_of(int k) {
 }
 
 // ---------------------------------------------------------------------------------------
+// plane-sphere maps (sect. 3): one array in, one array out, 8 B per cell.  map1_vec4 handles
+// the 16-byte aligned body, map1_scalar head, tail and misaligned ranges.
+// ---------------------------------------------------------------------------------------
+struct SphereSolveFastOp {
+    static __device__ __forceinline__ F2 apply2(F2 v) { return sphere_solve_pair_fast(v); }
+};
+struct SphereSolveOp {
+    static __device__ __forceinline__ F2 apply2(F2 v) {
+        return F2{sphere_solve_cell(v.x), sphere_solve_cell(v.y)};
+    }
+};
+struct SphereVolumeOp {
+    static __device__ __forceinline__ F2 apply2(F2 v) { return sphere_volume_pair(v); }
+};
+
+template <class OP>
+__global__ void __launch_bounds__(kBlock)
+map1_vec4(const float4 *__restrict__ in, float4 *__restrict__ out, int64_t n4) {
+    const int64_t stride = (int64_t)gridDim.x * kBlock;
+    for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < n4; i += stride) {
+        const float4 v = ld_stream(in + i);
+        const F2 lo = OP::apply2(F2{v.x, v.y}), hi = OP::apply2(F2{v.z, v.w});
+        st_stream(out + i, make_float4(lo.x, lo.y, hi.x, hi.y));
+    }
+}
+template <class OP>
+__global__ void __launch_bounds__(kBlock)
+map1_scalar(const float *__restrict__ in, float *__restrict__ out, int64_t head, int64_t tail0,
+            int64_t N) {
+    const int64_t stride = (int64_t)gridDim.x * kBlock;
+    const int64_t count = head + (N - tail0);
+    for (int64_t j = (int64_t)blockIdx.x * kBlock + threadIdx.x; j < count; j += stride) {
+        const int64_t i = j < head ? j : tail0 + (j - head);
+        const float v = in[i];
+        out[i] = OP::apply2(F2{v, v}).x;
+    }
+}
+
+template <class OP>
+static int launch_map1(const float *in, float *out, int64_t N, cudaStream_t stream) {
+    if (N < 0) return PLIC_ERR_SIZE;
+    if (N == 0) return PLIC_OK;
+    if (!in || !out) return PLIC_ERR_NULL;
+    const uintptr_t pi = (uintptr_t)in, po = (uintptr_t)out;
+    if ((pi | po) & 3u) return PLIC_ERR_ALIGN;
+    cudaError_t err;
+    const DeviceInfo *info = device_info(&err);
+    if (!info) return PLIC_ERR_LAUNCH;
+    int64_t head = (pi & 15u) == (po & 15u) ? (int64_t)(((16u - (pi & 15u)) & 15u) >> 2) : N;
+    if (head > N) head = N;
+    const int64_t n4 = (N - head) / 4;
+    const int64_t tail0 = head + 4 * n4;
+    const int64_t full = (int64_t)info->sms * 8;                     // 8 resident blocks of 256
+    if (n4 > 0) {
+        const int64_t need = (n4 + kBlock - 1) / kBlock;
+        map1_vec4<OP><<<(int)(need < full ? need : full), kBlock, 0, stream>>>(
+            (const float4 *)(in + head), (float4 *)(out + head), n4);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+    }
+    const int64_t rest = head + (N - tail0);
+    if (rest > 0) {
+        const int64_t need = (rest + kBlock - 1) / kBlock;
+        map1_scalar<OP><<<(int)(need < full ? need : full), kBlock, 0, stream>>>(in, out, head,
+                                                                                 tail0, N);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+    }
+    return cudaGetLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
+}
+
+// ---------------------------------------------------------------------------------------
 // host-array API: chunked, three-stage pipeline (H2D | kernel | D2H) over three streams
 // ---------------------------------------------------------------------------------------
 constexpr int kSlots = 3;
@@ -527,6 +597,16 @@ int plic_roundtrip_error(const float *nx, const float *ny, const float *nz, floa
         nx, ny, nz, E, N, L);
     plic::g_launches.fetch_add(1, std::memory_order_relaxed);
     return cudaGetLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
+}
+
+int plic_sphere_solve(const float *V0, float *d0, int64_t N, int fast, cudaStream_t stream) {
+    if (fast != 0 && fast != PLIC_FAST) return PLIC_ERR_METHOD;
+    return fast ? plic::launch_map1<plic::SphereSolveFastOp>(V0, d0, N, stream)
+                : plic::launch_map1<plic::SphereSolveOp>(V0, d0, N, stream);
+}
+
+int plic_sphere_volume(const float *d0, float *V0, int64_t N, cudaStream_t stream) {
+    return plic::launch_map1<plic::SphereVolumeOp>(d0, V0, N, stream);
 }
 
 int plic_solve_host(const float *V0, const float *nx, const float *ny, const float *nz,

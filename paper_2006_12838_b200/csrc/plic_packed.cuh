@@ -393,4 +393,49 @@ __device__ __forceinline__ F2 volume_pair(F2 d0, F2 nx, F2 ny, F2 nz) {
     return sel2(gt2(d0, f2(0.0f)), Vc, V);                                       // eq. (6)
 }
 
+// ---------------------------------------------------------------------------------------
+// plane-sphere intersection (sect. 3): unit-volume sphere, r = (3/(4 pi))^(1/3)
+// (eq. (34)).  Forward eq. (37) in cap form: with a = r - |d0| the smaller cap has volume
+// pi/3 a^2 (3r - a), mirrored for d0 > 0 -- the same polynomial as eq. (37), evaluated from the
+// near pole so that both ends keep full relative accuracy.
+// Inverse eq. (38): atan2(2 sqrt(V0 - V0^2), 2 V0 - 1) = acos(2 V0 - 1) because the two arguments
+// lie on the unit circle.  With V = min(V0, 1 - V0) and psi = asin(sqrt V)/3 in [0, pi/12]
+// (acos(1 - 2V) = 2 asin(sqrt V)) the cap height is
+//   a = r - |d0| = 2r (sin(pi/6) - sin(pi/6 - 2 psi)) = 4r sin(psi) cos(pi/6 - psi),
+// which has no cancellation at V -> 0 (eq. (38) as printed loses the digits of V0 in 2 V0 - 1).
+// sin(psi) = g(sqrt V) is the same sin(asin(C)/3) as in cases (3)/(4) of the cube, C <= 0.7072.
+// ---------------------------------------------------------------------------------------
+constexpr float kSphereR = 0.62035048f;                 // fp32((3/(4 pi))^(1/3)), eq. (34)
+constexpr float kSphereRlo = 1.08197492e-8f;            // r - kSphereR: keeps small caps accurate
+
+__device__ __forceinline__ F2 sphere_volume_pair(F2 d0) {
+    const F2 ad = abs2(d0);
+    // a = r - |d0|: the difference with fp32(r) is exact near the pole, the tail of r is added after
+    const F2 a = F2{fmaxf((kSphereR - ad.x) + kSphereRlo, 0.0f), fmaxf((kSphereR - ad.y) + kSphereRlo, 0.0f)};
+    // pi/3 a^2 (3r - a)
+    const F2 V = mul2(mul2(a, a), fma2(a, -1.04719755f, f2(3.0f * kSphereR * 1.04719755f)));
+    return sel2(gt2(d0, f2(0.0f)), fma2(V, -1.0f, f2(1.0f)), V);
+}
+
+__device__ __forceinline__ F2 sphere_solve_pair_fast(F2 V0) {
+    const F2 V = sat2(min2(V0, fma2(V0, -1.0f, f2(1.0f))));
+    const F2 nsin = neg_sin_third_asin_fast2(sqrt2(V));                          // -sin(psi)
+    const F2 cosp = sqrt2(fma2(mul2(nsin, -1.0f), nsin, f2(1.0f)));              // cos(psi)
+    // a = 4r sin(psi) (sqrt(3)/2 cos(psi) + 1/2 sin(psi))
+    const F2 a = mul2(mul2(nsin, -4.0f * kSphereR), fma2(cosp, 0.866025404f, mul2(nsin, -0.5f)));
+    const F2 r = F2{fmaxf(kSphereR - a.x, 0.0f), fmaxf(kSphereR - a.y, 0.0f)};
+    const F2 t = fma2(V0, -1.0f, f2(0.5f));
+    return F2{__uint_as_float(__float_as_uint(r.x) | (~__float_as_uint(t.x) & 0x80000000u)),
+              __uint_as_float(__float_as_uint(r.y) | (~__float_as_uint(t.y) & 0x80000000u))};
+}
+
+// precise: IEEE sqrt, libm asin/sin/cos
+__device__ __forceinline__ float sphere_solve_cell(float V0) {
+    const float V = fmaxf(fminf(V0, 1.0f - V0), 0.0f);
+    const float psi = asinf(fminf(sqrtf(V), 1.0f)) * (1.0f / 3.0f);
+    const float a = 4.0f * kSphereR * sinf(psi) * cosf(0.523598776f - psi);
+    const float r = fmaxf(kSphereR - a, 0.0f);
+    return V0 > 0.5f ? r : -r;
+}
+
 }  // namespace plic

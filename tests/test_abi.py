@@ -25,7 +25,8 @@ def _declared_functions():
 
 def test_header_declares_the_boundary():
     names = _declared_functions()
-    for must in ("plic_solve", "plic_volume", "plic_roundtrip_error", "plic_solve_host", "plic_volume_host",
+    for must in ("plic_solve", "plic_volume", "plic_roundtrip_error", "plic_sphere_solve",
+                 "plic_sphere_volume", "plic_solve_host", "plic_volume_host",
                  "plic_method_name", "plic_version", "plic_launch_count"):
         assert must in names
 
@@ -91,6 +92,13 @@ def test_argument_validation_needs_no_device(plic):
     assert lib.plic_roundtrip_error(p, p, p, p, 4, 256, 9, None) == -3
     assert lib.plic_roundtrip_error(p, p, None, p, 4, 256, 0x40, None) == -1
     assert lib.plic_solve(p, p, p, p, p, 4, 0x40, None) == -3
+    # plane-sphere entry points
+    assert lib.plic_sphere_solve(None, None, 0, 0, None) == 0
+    assert lib.plic_sphere_solve(p, p, -1, 0, None) == -2
+    assert lib.plic_sphere_solve(p, None, 4, 0, None) == -1
+    assert lib.plic_sphere_solve(p, p, 4, 1, None) == -3
+    assert lib.plic_sphere_volume(None, p, 4, None) == -1
+    assert lib.plic_sphere_volume(ctypes.c_void_p(p.value + 2), p, 1, None) == -5
     # misaligned (not a multiple of 4 bytes)
     q = ctypes.c_void_p(p.value + 2)
     assert lib.plic_solve(q, p, p, p, p, 1, 0, None) == -5
