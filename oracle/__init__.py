@@ -12,7 +12,8 @@ lives entirely in the C file, whose header cites the paper passages it follows
     case(d0, nx, ny, nz)   -> 1..5    intersection case of eq. (11)
 
 Sub-modules (numpy fp64, same rules): ``oracle.sphere`` -- the plane-sphere problem of sect. 3
-(eq. (37) and its inverse by bisection).
+(eq. (37) and its inverse by bisection); ``oracle.curvature`` -- the curvature calculation of
+sect. 4 / appendix B (PY normal, PLIC point neighbourhood, paraboloid fit, eq. (63)).
 """
 from __future__ import annotations
 
