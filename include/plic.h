@@ -135,6 +135,33 @@ int plic_sphere_solve(const float *V0, float *d0, int64_t N, int fast, cudaStrea
 int plic_sphere_volume(const float *d0, float *V0, int64_t N, cudaStream_t stream);
 
 /*
+ * plic_curvature -- mean curvature of the interface from fill levels (sect. 4 and appendix B,
+ * PAPER.md:323-393, 510-614; eq. (41): phi_0..phi_26 -> kappa).  For every interface lattice point
+ * (0 < phi < 1) with a full 3^3 neighbourhood: Parker-Youngs normal (eq. (54), (55)), basis
+ * (eq. (42)-(45)), PLIC-corrected neighbour points (eq. (46), analytic PLIC solve with the centre's
+ * normal, interface neighbours only), least-squares paraboloid (eq. (47)-(49), (69), (70); with k < 5
+ * points only the first k of (A, B, C, H, I) are fitted), kappa by eq. (63).
+ *
+ *   phi      DEVICE pointer, fp32, nx*ny*nz fill levels, index x + nx (y + ny z), read only.
+ *   kappa    DEVICE pointer, fp32, same shape, written: eq. (63) at interface points, 0 at every
+ *            other cell (also at interface points on the lattice border, with a vanishing
+ *            gradient sum, or without interface neighbours).  Must not overlap phi.
+ *   work     DEVICE pointer to work_entries int32 of scratch owned by the caller.  On return
+ *            (after the stream has run) work[0] = number of interface points found and
+ *            work[1..] their cell indices, in no particular order.  work_entries >= 1 + that
+ *            number is required for a complete result (1 + nx*ny*nz always suffices); points
+ *            beyond the capacity keep kappa = 0, which the caller can detect from work[0].
+ *   nx, ny, nz >= 0, nx*ny*nz < 2^31.
+ *
+ * Sign: with the normal of eq. (54) pointing out of the fluid, eq. (63) is negative for a convex
+ * fluid body (-1/R for a drop of radius R) and positive for a bubble.
+ * Two kernels are enqueued on `stream` (a streaming pass and a dense pass over the interface
+ * list); errors, ownership and stream semantics as plic_solve.
+ */
+int plic_curvature(const float *phi, float *kappa, int nx, int ny, int nz, int32_t *work,
+                   int64_t work_entries, cudaStream_t stream);
+
+/*
  * plic_solve_host / plic_volume_host -- the same maps for HOST arrays (pageable or pinned;
  * pinned memory makes the copies asynchronous).  The range is cut into chunks; host->device
  * copies, the kernel and the device->host copy of consecutive chunks overlap on three

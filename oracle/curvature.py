@@ -127,6 +127,35 @@ def curvature_cells(phi27: np.ndarray, r=R_VEC) -> np.ndarray:
     return kappa
 
 
+def fit_diagnostics(phi27: np.ndarray, r=R_VEC):
+    """Test diagnostics, not part of the method: per cell the number of interface neighbours, the
+    2-norm condition number of the k x k system of eq. (70) (inf where there is none) and its
+    smallest eigenvalue (0 where there is none)."""
+    phi27 = np.asarray(phi27, dtype=np.float64)
+    n = py_normal(phi27)
+    nb = np.array([i for i in range(27) if i != CENTRE])
+    use = ((phi27[:, nb] > 0.0) & (phi27[:, nb] < 1.0)).astype(np.float64)
+    count = use.sum(axis=1).astype(int)
+    cond = np.full(phi27.shape[0], np.inf)
+    lam_min = np.zeros(phi27.shape[0])
+    good = ((n * n).sum(axis=1) > 0.0) & (count > 0)
+    if good.any():
+        bx, by, _ = basis(n[good], r)
+        e = E[nb]
+        x, y = bx @ e.T, by @ e.T
+        Q = np.stack([x * x, y * y, x * y, x, y], axis=2) * use[good][:, :, None]
+        M = np.einsum("mia,mib->mab", Q, Q)
+        c = np.empty(M.shape[0])
+        lm = np.empty(M.shape[0])
+        for j, k in enumerate(np.minimum(count[good], 5)):
+            ev = np.linalg.eigvalsh(M[j, :k, :k])
+            lm[j] = max(ev[0], 0.0)
+            c[j] = ev[-1] / ev[0] if ev[0] > 0.0 else np.inf
+        cond[good] = c
+        lam_min[good] = lm
+    return count, cond, lam_min
+
+
 def gather27(phi: np.ndarray, idx: np.ndarray) -> np.ndarray:
     """The 3^3 neighbourhoods (ordering of E) of the interior cells idx = [m, 3] as (z, y, x)."""
     out = np.empty((idx.shape[0], 27))

@@ -14,6 +14,8 @@ shared library is missing it is built with nvcc, and if that fails the import ra
                                             the paper's benchmark loop, eq. (31)-(33)
     plic_sphere_solve(V0, out=None, fast=False) -> d0, plic_sphere_volume(d0, out=None) -> V0
                                             the plane-sphere intersection of sect. 3
+    plic_curvature(phi, out=None, work=None) -> kappa
+                                            curvature from a lattice of fill levels, sect. 4
 """
 from __future__ import annotations
 
@@ -23,7 +25,8 @@ import os
 from . import build as _build
 
 __all__ = ["METHODS", "FAST", "BLANK", "method_id", "plic_solve", "plic_volume",
-           "plic_roundtrip_error", "plic_sphere_solve", "plic_sphere_volume", "plic_solve_host",
+           "plic_roundtrip_error", "plic_sphere_solve", "plic_sphere_volume", "plic_curvature",
+           "plic_solve_host",
            "plic_volume_host", "plic_host_release", "plic_method_name", "plic_error_string",
            "plic_version", "plic_launch_config", "plic_launch_count", "PlicError", "lib",
            "LIB_PATH"]
@@ -57,6 +60,9 @@ def _load() -> ctypes.CDLL:
     lib_.plic_sphere_solve.restype = ctypes.c_int
     lib_.plic_sphere_volume.argtypes = [fp, fp, i64, ctypes.c_void_p]
     lib_.plic_sphere_volume.restype = ctypes.c_int
+    lib_.plic_curvature.argtypes = [fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, i64,
+                                    ctypes.c_void_p]
+    lib_.plic_curvature.restype = ctypes.c_int
     lib_.plic_solve_host.argtypes = [fp, fp, fp, fp, fp, i64, ctypes.c_int]
     lib_.plic_solve_host.restype = ctypes.c_int
     lib_.plic_volume_host.argtypes = [fp, fp, fp, fp, fp, i64]
@@ -213,6 +219,32 @@ def plic_sphere_volume(d0, out=None, stream=None):
                                     _stream_handle(stream, d0.device))
     if rc != 0:
         raise PlicError(rc, "plic_sphere_volume")
+    return out
+
+
+def plic_curvature(phi, out=None, work=None, stream=None):
+    """kappa (eq. (63)) on a lattice of fill levels phi[z, y, x] (3-D contiguous float32 CUDA
+    tensor); `work` is an int32 CUDA tensor of scratch (default: 1 + phi.numel() entries).
+    Returns `out`; work[0] then holds the number of interface points."""
+    import torch
+    if not (phi.is_cuda and phi.dtype == torch.float32 and phi.dim() == 3 and phi.is_contiguous()):
+        raise ValueError("phi must be a contiguous 3-D float32 CUDA tensor [nz, ny, nx]")
+    if out is None:
+        out = torch.empty_like(phi)
+    elif not (out.is_cuda and out.dtype == torch.float32 and out.is_contiguous()
+              and out.shape == phi.shape and out.device == phi.device):
+        raise ValueError("out must be a contiguous float32 CUDA tensor of phi's shape")
+    if work is None:
+        work = torch.empty(1 + phi.numel(), dtype=torch.int32, device=phi.device)
+    elif not (work.is_cuda and work.dtype == torch.int32 and work.is_contiguous()
+              and work.device == phi.device):
+        raise ValueError("work must be a contiguous int32 CUDA tensor")
+    nz, ny, nx = phi.shape
+    with torch.cuda.device(phi.device):
+        rc = lib.plic_curvature(phi.data_ptr(), out.data_ptr(), nx, ny, nz, work.data_ptr(),
+                                work.numel(), _stream_handle(stream, phi.device))
+    if rc != 0:
+        raise PlicError(rc, "plic_curvature")
     return out
 
 

@@ -21,6 +21,7 @@
 #include "../../include/plic.h"
 #include "plic_methods.cuh"
 #include "plic_packed.cuh"
+#include "plic_curvature.cuh"
 
 #define PLIC_VERSION 100
 
@@ -607,6 +608,33 @@ int plic_sphere_solve(const float *V0, float *d0, int64_t N, int fast, cudaStrea
 
 int plic_sphere_volume(const float *d0, float *V0, int64_t N, cudaStream_t stream) {
     return plic::launch_map1<plic::SphereVolumeOp>(d0, V0, N, stream);
+}
+
+int plic_curvature(const float *phi, float *kappa, int nx, int ny, int nz, int32_t *work,
+                   int64_t work_entries, cudaStream_t stream) {
+    if (nx < 0 || ny < 0 || nz < 0) return PLIC_ERR_SIZE;
+    const int64_t ncells = (int64_t)nx * ny * nz;
+    if (ncells > 0x7fffffffLL) return PLIC_ERR_SIZE;
+    if (ncells == 0) return PLIC_OK;
+    if (!phi || !kappa || !work) return PLIC_ERR_NULL;
+    if (work_entries < 2) return PLIC_ERR_SIZE;
+    if (((uintptr_t)phi | (uintptr_t)kappa | (uintptr_t)work) & 3u) return PLIC_ERR_ALIGN;
+    cudaError_t err;
+    const plic::DeviceInfo *info = plic::device_info(&err);
+    if (!info) return PLIC_ERR_LAUNCH;
+    int64_t cap64 = work_entries - 1;
+    if (cap64 > ncells) cap64 = ncells;
+    const int capacity = (int)cap64;
+    if (cudaMemsetAsync(work, 0, sizeof(int32_t), stream) != cudaSuccess) return PLIC_ERR_LAUNCH;
+    int64_t need = (ncells + 255) / 256, full = (int64_t)info->sms * 8;
+    plic::curv_mark<<<(int)(need < full ? need : full), 256, 0, stream>>>(phi, kappa, nx, ny, nz,
+                                                                         work, capacity);
+    need = ((int64_t)capacity + plic::kCurvBlock - 1) / plic::kCurvBlock;
+    full = (int64_t)info->sms * 32;
+    plic::curv_cells<<<(int)(need < full ? need : full), plic::kCurvBlock, 0, stream>>>(
+        phi, kappa, nx, ny, work, capacity);
+    plic::g_launches.fetch_add(2, std::memory_order_relaxed);
+    return cudaGetLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
 }
 
 int plic_solve_host(const float *V0, const float *nx, const float *ny, const float *nz,

@@ -26,7 +26,7 @@ def _declared_functions():
 def test_header_declares_the_boundary():
     names = _declared_functions()
     for must in ("plic_solve", "plic_volume", "plic_roundtrip_error", "plic_sphere_solve",
-                 "plic_sphere_volume", "plic_solve_host", "plic_volume_host",
+                 "plic_sphere_volume", "plic_curvature", "plic_solve_host", "plic_volume_host",
                  "plic_method_name", "plic_version", "plic_launch_count"):
         assert must in names
 
@@ -99,6 +99,12 @@ def test_argument_validation_needs_no_device(plic):
     assert lib.plic_sphere_solve(p, p, 4, 1, None) == -3
     assert lib.plic_sphere_volume(None, p, 4, None) == -1
     assert lib.plic_sphere_volume(ctypes.c_void_p(p.value + 2), p, 1, None) == -5
+    # plic_curvature
+    assert lib.plic_curvature(None, None, 0, 5, 5, None, 0, None) == 0
+    assert lib.plic_curvature(p, p, -1, 5, 5, p, 8, None) == -2
+    assert lib.plic_curvature(p, p, 2048, 2048, 2048, p, 8, None) == -2      # >= 2^31 cells
+    assert lib.plic_curvature(p, p, 2, 2, 2, None, 8, None) == -1
+    assert lib.plic_curvature(p, p, 2, 2, 2, p, 1, None) == -2
     # misaligned (not a multiple of 4 bytes)
     q = ctypes.c_void_p(p.value + 2)
     assert lib.plic_solve(q, p, p, p, p, 1, 0, None) == -5

@@ -1,0 +1,150 @@
+"""GPU parity of plic_curvature (sect. 4 / appendix B) against oracle/curvature.py, cell by cell
+through the C ABI.
+
+Tolerance: the fitted parameters are x = M^-1 b.  The fp32 path
+perturbs the heights z_i of eq. (46) by <= ~1e-6 (PLIC solve), i.e. b by ~1e-6 |Q|, and rounds M to
+~1e-7 |M|, so |dx| <= |M^-1| (|db| + |dM| |x|) and, kappa being essentially A + B,
+  |kappa - ref| <= TOL_K * max(1, 1/lambda_min(M)) * max(1, cond(M)/100) * max(1, |ref|),  TOL_K = 5e-6.
+On smooth bodies lambda_min is about 2 and cond(M) 10-20, where this is the plain 5e-6."""
+import os
+import sys
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import curvature as oc
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+import lattices  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+TOL_K = 5e-6
+
+
+@pytest.fixture(scope="module")
+def plic():
+    import paper_2006_12838_b200 as p
+    return p
+
+
+def tolerance(cond, lam_min, ref):
+    return (TOL_K * np.maximum(1.0, 1.0 / np.maximum(lam_min, 1e-30)) * np.maximum(1.0, cond / 100.0)
+            * np.maximum(1.0, np.abs(ref)))
+
+
+def run_gpu(plic, phi, work_entries=None):
+    t = torch.from_numpy(np.ascontiguousarray(phi)).cuda()
+    work = None if work_entries is None else torch.empty(work_entries, dtype=torch.int32, device="cuda")
+    before = plic.plic_launch_count()
+    if work is None:
+        work = torch.empty(1 + t.numel(), dtype=torch.int32, device="cuda")
+    k = plic.plic_curvature(t, work=work)
+    torch.cuda.synchronize()
+    assert plic.plic_launch_count() == before + 2
+    return k.cpu().numpy(), work.cpu().numpy()
+
+
+def check(plic, phi, what, min_cells=100):
+    ref = oc.curvature_lattice(phi)
+    got, work = run_gpu(plic, phi)
+    assert got.shape == phi.shape and got.dtype == np.float32
+    inner = np.zeros(phi.shape, dtype=bool)
+    inner[1:-1, 1:-1, 1:-1] = True
+    iface = (phi > 0) & (phi < 1) & inner
+    idx = np.argwhere(iface)
+    assert len(idx) >= min_cells, what
+    # the interface list: every interior interface point exactly once
+    assert work[0] == len(idx)
+    lin = idx[:, 2] + phi.shape[2] * (idx[:, 1] + phi.shape[1] * idx[:, 0])
+    assert np.array_equal(np.sort(work[1:1 + work[0]]), np.sort(lin))
+    # zero everywhere else, bit for bit
+    assert np.all(got[~iface] == 0.0)
+    count, cond, lam = oc.fit_diagnostics(oc.gather27(phi.astype(np.float64), idx))
+    r = ref[iface]
+    g = got[iface].astype(np.float64)
+    ok = np.isfinite(r) & np.isfinite(cond) & (cond < 1e6)
+    assert ok.mean() > 0.95, what
+    tol = tolerance(cond[ok], lam[ok], r[ok])
+    err = np.abs(g[ok] - r[ok])
+    j = int(np.argmax(err / tol))
+    assert np.all(err <= tol), "%s: |dk| %.3e (tol %.3e, cond %.2e, count %d, ref %.5f)" % (
+        what, err[j], tol[j], cond[ok][j], count[ok][j], r[ok][j])
+    assert np.all(np.isfinite(g[ok]))
+    return g, r, ok
+
+
+def test_spheres(plic):
+    for R, L in ((8, 24), (12, 33), (24, 56)):
+        phi = lattices.sphere((L, L + 1, L + 3), (L / 2 + 0.8, L / 2 + 0.2, L / 2 + 0.1), R)
+        g, r, ok = check(plic, phi, "sphere R=%d" % R, 1000)
+        kk = -g[ok] * R
+        assert abs(kk.mean() - 1.0) < 0.02 and np.abs(kk - 1.0).mean() < 0.08     # eq. (50)
+
+
+def test_bubble_cylinder_planes(plic):
+    phi = (1.0 - lattices.sphere((32, 32, 32), (16.2, 15.9, 16.4), 12)).astype(np.float32)
+    g, r, ok = check(plic, phi, "bubble", 1000)
+    assert abs(g[ok].mean() * 12 - 1.0) < 0.02
+    g, r, ok = check(plic, lattices.cylinder((12, 40, 40), (20.3, 19.8), 14), "cylinder", 1000)
+    assert abs(-g[ok].mean() * 14 - 0.5) < 0.02
+    for normal, off in (((1, 0, 0), 7.3), ((1, 1, 0), 14.2), ((1, -1, 1), 5.1), ((0.3, 0.5, 0.81), 12.9)):
+        g, r, ok = check(plic, lattices.plane((14, 15, 16), normal, off), "plane %r" % (normal,), 50)
+        if normal != (0.3, 0.5, 0.81):
+            assert np.max(np.abs(g[ok])) < 1e-5
+
+
+def test_small_drops_reduced_rank_and_noise(plic):
+    # a random three-phase lattice (45 % gas, 45 % fluid, 10 % interface points): the normal is
+    # shaped by the fluid/gas cells, interface neighbours are few (k < 5 parameters are fitted)
+    # and sit in general position
+    rng = np.random.Generator(np.random.Philox(key=41))
+    u = rng.random((40, 40, 40))
+    phi = np.where(u < 0.45, 0.0, np.where(u < 0.9, 1.0, rng.uniform(0.05, 0.95, u.shape))).astype(np.float32)
+    ref = oc.curvature_lattice(phi)
+    got, work = run_gpu(plic, phi)
+    inner = np.zeros(phi.shape, dtype=bool)
+    inner[1:-1, 1:-1, 1:-1] = True
+    iface = (phi > 0) & (phi < 1) & inner
+    assert work[0] == iface.sum()
+    count, cond, lam = oc.fit_diagnostics(oc.gather27(phi.astype(np.float64), np.argwhere(iface)))
+    # |kappa| > 10 per cell is a fit through nearly coincident abscissae, not a curvature: excluded
+    ok = np.isfinite(ref[iface]) & (cond < 1e6) & (np.abs(ref[iface]) < 10.0)
+    for k in (1, 2, 3, 4):
+        assert ((count == k) & ok).sum() >= 20, k                         # reduced rank is exercised
+    assert np.all(got[iface][count == 0] == 0)                            # no interface neighbour (C2)
+    tol = tolerance(cond[ok], lam[ok], ref[iface][ok])
+    err = np.abs(got[iface][ok] - ref[iface][ok])
+    j = int(np.argmax(err / tol))
+    assert np.all(err <= tol), (err[j], tol[j], cond[ok][j], count[ok][j], ref[iface][ok][j])
+    # noisy interface sheet
+    phi = lattices.plane((20, 20, 20), (0.2, 0.3, 1.0), 9.7)
+    noisy = np.where((phi > 0) & (phi < 1), np.clip(phi + rng.uniform(-0.2, 0.2, phi.shape), 0.01, 0.99), phi)
+    check(plic, noisy.astype(np.float32), "noisy sheet", 300)
+
+
+def test_shapes_borders_capacity_empty(plic):
+    # no interior: every dimension < 3
+    for shape in ((1, 1, 1), (2, 5, 7), (5, 2, 7), (7, 5, 2)):
+        phi = np.full(shape, 0.5, dtype=np.float32)
+        got, work = run_gpu(plic, phi)
+        assert np.all(got == 0) and work[0] == 0
+    # all-interface lattice with constant phi: gradient sum vanishes -> 0 (C2)
+    phi = np.full((6, 6, 6), 0.5, dtype=np.float32)
+    got, work = run_gpu(plic, phi)
+    assert np.all(got == 0) and work[0] == 4 ** 3
+    # interface cut by the lattice border: border cells stay 0
+    phi = lattices.sphere((16, 16, 16), (8, 8, 2.0), 6)
+    got, _ = run_gpu(plic, phi)
+    assert np.all(got[0] == 0) and np.all(got[:, 0] == 0) and np.all(got[:, :, -1] == 0)
+    # work too small: the count is still reported, the listed cells are computed, the rest stay 0
+    phi = lattices.sphere((24, 24, 24), (12.3, 11.7, 12.1), 8)
+    full, work_full = run_gpu(plic, phi)
+    part, work = run_gpu(plic, phi, work_entries=101)
+    assert work[0] == work_full[0] > 100
+    done = part != 0
+    assert 0 < done.sum() <= 100 and np.array_equal(part[done], full[done])
+    # empty lattice
+    t = torch.zeros((0, 4, 4), device="cuda")
+    assert plic.plic_curvature(t).shape == (0, 4, 4)
