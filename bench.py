@@ -392,6 +392,30 @@ def run_ours(args):
     for k, v in methods.items():
         v["roofline_frac"] = v["hbm_gbs_per_gpu"] / peak
 
+    # ---- curvature on configs[4]: 256^3 lattice, sphere R = 60 (sect. 4; two launches per call) ----
+    curv = None
+    if not args.no_curvature:
+        R5 = 60.0
+        phi5 = torch.from_numpy(gen.sphere_fill_lattice(256, R5, (128.3, 127.7, 128.1), 8)).cuda()
+        kap5 = torch.empty_like(phi5)
+        work5 = torch.empty(1 + phi5.numel(), dtype=torch.int32, device="cuda")
+        c0 = plic.plic_launch_count()
+        ms, _ = time_launches(lambda: plic.plic_curvature(phi5, out=kap5, work=work5), args.steps,
+                              args.warmup, stream)
+        per_call = (plic.plic_launch_count() - c0) / (args.steps + args.warmup)
+        ms = max_over_ranks(ms) / args.steps
+        n_if = int(work5[0].item())
+        kk = -kap5[kap5 != 0].double() * R5
+        curv = {"workload": "configs[4]: 256^3 lattice, sphere R=60 at (128.3,127.7,128.1), phi = fraction "
+                            "of 8^3 sub-cell points inside", "ms_per_call": ms, "launches_per_call": per_call,
+                "lattice_gcells_per_s": phi5.numel() / (ms * 1e-3) / 1e9, "interface_points": n_if,
+                "interface_mpoints_per_s": n_if / (ms * 1e-3) / 1e6,
+                "hbm_gbs": 8 * phi5.numel() / (ms * 1e-3) / 1e9,
+                "roofline_frac": 8 * phi5.numel() / (ms * 1e-3) / 1e9 / measured_peak()[0],
+                "bytes_per_lattice_cell": 8, "minus_kappa_R_mean": float(kk.mean()),
+                "L1_error_eq50": float((kk - 1.0).abs().mean())}
+        del phi5, kap5, work5
+
     # ---- end to end through the host-array C ABI: pinned host buffers, copies inside ----------
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     pin = [torch.from_numpy(a).pin_memory() for a in host]
@@ -444,6 +468,8 @@ def run_ours(args):
         }
         if paper is not None:
             line["paper_benchmark"] = paper
+        if curv is not None:
+            line["curvature"] = curv
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(host)
         print(json.dumps(line), flush=True)
@@ -465,6 +491,7 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--prewarm-ms", type=float, default=300.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-curvature", action="store_true", help="skip the plic_curvature leg")
     ap.add_argument("--paper-log2n", type=int, default=24,
                     help="normals in the paper-shaped compute-bound leg = 2^k, L = 256 volumes each "
                          "(the paper: k = 26); 0 skips it")

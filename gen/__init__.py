@@ -16,8 +16,9 @@ in DESIGN.md.
 """
 from .workloads import (CHUNK, random_sphere, edge_cells, config1, snapped_beta,
                         paper_benchmark_set, paper_normals, roundtrip_volumes, sphere_lattice,
+                        sphere_fill_lattice,
                         shard_range)
 
 __all__ = ["CHUNK", "random_sphere", "edge_cells", "config1", "snapped_beta",
-           "paper_benchmark_set", "paper_normals", "roundtrip_volumes", "sphere_lattice",
+           "paper_benchmark_set", "paper_normals", "roundtrip_volumes", "sphere_lattice", "sphere_fill_lattice",
            "shard_range"]

@@ -245,6 +245,19 @@ def sphere_lattice(L: int = 256, R: float = 60.0, centre=(128.3, 127.7, 128.1), 
             "R": float(R), "centre": tuple(float(x) for x in o)}
 
 
+def sphere_fill_lattice(L: int = 256, R: float = 60.0, centre=(128.3, 127.7, 128.1), sub: int = 8):
+    """Config 5 as a full lattice for plic_curvature: phi[z, y, x] (fp32, L^3), 1 inside the sphere,
+    0 outside, and on the interface the sampled fraction of sphere_lattice() (same convention)."""
+    cells = sphere_lattice(L, R, centre, sub)
+    o = np.asarray(centre, dtype=np.float64)
+    ax = np.arange(L, dtype=np.float64) + 0.5
+    r2 = ((ax - o[2]) ** 2)[:, None, None] + ((ax - o[1]) ** 2)[None, :, None] + ((ax - o[0]) ** 2)[None, None, :]
+    phi = (r2 < R * R).astype(np.float32)
+    ijk = cells["ijk"]
+    phi[ijk[:, 2], ijk[:, 1], ijk[:, 0]] = cells["phi"]
+    return phi
+
+
 def shard_range(N: int, rank: int, world: int, align: int = 32):
     """Contiguous [lo, hi) of N cells owned by `rank` of `world` ranks; interior
     boundaries are multiples of `align` cells so every shard keeps the 128-byte

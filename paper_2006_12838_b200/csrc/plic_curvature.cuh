@@ -13,9 +13,9 @@
 //
 // Two kernels, because interface points are a 2-D surface in a 3-D lattice (0.4 % of the cells of
 // a 256^3 box holding an R = 60 drop):
-//   curv_mark   streams the lattice once (HBM bound: 4 B read + 4 B written per cell), writes
+//   curv_mark4  streams the lattice once (HBM bound: 4 B read + 4 B written per cell), writes
 //               kappa = 0 everywhere and appends the index of every interior interface point to a
-//               list (one atomicAdd per warp);
+//               list (one atomicAdd per warp); curv_mark is its scalar form for misaligned lattices;
 //   curv_cells  one thread per list entry, so warps are dense: gathers the 27 fill levels (L2
 //               hits, the lattice has just been streamed), and runs steps 1-6 in registers; the 26
 //               neighbour solves go through the packed two-cells-per-instruction analytic solver.
@@ -27,6 +27,15 @@
 namespace plic {
 
 constexpr int kCurvBlock = 64;                 // threads per block of curv_cells
+
+__device__ __forceinline__ bool curv_interior(int64_t i, int nx, int ny, int nz) {
+    const unsigned u = (unsigned)i;                               // ncells < 2^31: 32-bit divisions
+    const unsigned t = u / (unsigned)nx;
+    const int x = (int)(u - t * (unsigned)nx);
+    const int z = (int)(t / (unsigned)ny);
+    const int y = (int)(t - (unsigned)z * (unsigned)ny);
+    return x > 0 && x < nx - 1 && y > 0 && y < ny - 1 && z > 0 && z < nz - 1;
+}
 
 // ---- curv_mark -----------------------------------------------------------------------------
 // list[0] counts every interior interface point found (also beyond capacity); entries
@@ -43,12 +52,7 @@ curv_mark(const float *__restrict__ phi, float *__restrict__ kappa, int nx, int 
         if (i < ncells) {
             const float p = __ldg(phi + i);
             kappa[i] = 0.0f;
-            if (p > 0.0f && p < 1.0f) {
-                const int x = (int)(i % nx);
-                const int64_t t = i / nx;
-                const int y = (int)(t % ny), z = (int)(t / ny);
-                hit = x > 0 && x < nx - 1 && y > 0 && y < ny - 1 && z > 0 && z < nz - 1;
-            }
+            hit = p > 0.0f && p < 1.0f && curv_interior(i, nx, ny, nz);
         }
         const unsigned m = __ballot_sync(0xffffffffu, hit);
         if (m) {
@@ -58,6 +62,71 @@ curv_mark(const float *__restrict__ phi, float *__restrict__ kappa, int nx, int 
             const int slot = start + __popc(m & ((1u << lane) - 1u));
             if (hit && slot < capacity) list[1 + slot] = (int)i;
         }
+    }
+}
+
+// Vector form for 16-byte aligned lattices: four cells per thread and two such groups in flight
+// per thread (32 B loaded before anything is consumed); the ncells % 4 trailing cells are taken
+// by the first threads of block 0.  Same list semantics as curv_mark.
+__device__ __forceinline__ void curv_append(unsigned hits, int64_t first, int *__restrict__ list,
+                                            int capacity) {
+    // hits: bit c set = cell first + c is an interior interface point; warp-aggregated append
+    const int lane = threadIdx.x & 31;
+    const int mine = __popc(hits);
+    if (__ballot_sync(0xffffffffu, mine > 0) == 0) return;
+    int scan = mine;                                              // inclusive prefix sum over lanes
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, scan, d);
+        if (lane >= d) scan += v;
+    }
+    int start = 0;
+    if (lane == 31) start = atomicAdd(list, scan);
+    start = __shfl_sync(0xffffffffu, start, 31);
+    int slot = start + scan - mine;
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+        if (hits & (1u << c)) {
+            if (slot < capacity) list[1 + slot] = (int)(first + c);
+            ++slot;
+        }
+}
+
+__global__ void __launch_bounds__(256)
+curv_mark4(const float4 *__restrict__ phi, float4 *__restrict__ kappa, int nx, int ny, int nz,
+           int *__restrict__ list, int capacity) {
+    const int64_t ncells = (int64_t)nx * ny * nz;
+    const int64_t n4 = ncells / 4;
+    const int64_t stride = (int64_t)gridDim.x * 256;
+    const float4 zero4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    // whole warps iterate together (the append uses warp collectives): bound by the warp's first lane
+    for (int64_t base = (int64_t)blockIdx.x * 256 + (threadIdx.x & ~31); base < n4; base += 2 * stride) {
+        const int64_t g0 = base + (threadIdx.x & 31), g1 = g0 + stride;
+        const bool in0 = g0 < n4, in1 = g1 < n4;
+        float4 p0 = zero4, p1 = zero4;
+        if (in0) p0 = __ldg(phi + g0);
+        if (in1) p1 = __ldg(phi + g1);
+        if (in0) kappa[g0] = zero4;
+        if (in1) kappa[g1] = zero4;
+        const float v0[4] = {p0.x, p0.y, p0.z, p0.w}, v1[4] = {p1.x, p1.y, p1.z, p1.w};
+        unsigned h0 = 0, h1 = 0;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            if (v0[c] > 0.0f && v0[c] < 1.0f && curv_interior(4 * g0 + c, nx, ny, nz)) h0 |= 1u << c;
+            if (v1[c] > 0.0f && v1[c] < 1.0f && curv_interior(4 * g1 + c, nx, ny, nz)) h1 |= 1u << c;
+        }
+        curv_append(h0, 4 * g0, list, capacity);
+        curv_append(h1, 4 * g1, list, capacity);
+    }
+    if (blockIdx.x == 0 && threadIdx.x < 32) {                    // the ncells % 4 trailing cells
+        const int64_t i = 4 * n4 + threadIdx.x;
+        unsigned h = 0;
+        if (i < ncells) {
+            const float p = reinterpret_cast<const float *>(phi)[i];
+            reinterpret_cast<float *>(kappa)[i] = 0.0f;
+            if (p > 0.0f && p < 1.0f && curv_interior(i, nx, ny, nz)) h = 1u;
+        }
+        curv_append(h, i, list, capacity);
     }
 }
 

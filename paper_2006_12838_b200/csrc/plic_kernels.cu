@@ -626,9 +626,16 @@ int plic_curvature(const float *phi, float *kappa, int nx, int ny, int nz, int32
     if (cap64 > ncells) cap64 = ncells;
     const int capacity = (int)cap64;
     if (cudaMemsetAsync(work, 0, sizeof(int32_t), stream) != cudaSuccess) return PLIC_ERR_LAUNCH;
-    int64_t need = (ncells + 255) / 256, full = (int64_t)info->sms * 8;
-    plic::curv_mark<<<(int)(need < full ? need : full), 256, 0, stream>>>(phi, kappa, nx, ny, nz,
-                                                                         work, capacity);
+    int64_t need, full = (int64_t)info->sms * 8;
+    if ((((uintptr_t)phi | (uintptr_t)kappa) & 15u) == 0 && ncells >= 4) {
+        need = (ncells / 4 + 511) / 512;                             // two float4 groups per thread
+        plic::curv_mark4<<<(int)(need < full ? need : full), 256, 0, stream>>>(
+            (const float4 *)phi, (float4 *)kappa, nx, ny, nz, work, capacity);
+    } else {
+        need = (ncells + 255) / 256;
+        plic::curv_mark<<<(int)(need < full ? need : full), 256, 0, stream>>>(phi, kappa, nx, ny, nz,
+                                                                             work, capacity);
+    }
     need = ((int64_t)capacity + plic::kCurvBlock - 1) / plic::kCurvBlock;
     full = (int64_t)info->sms * 32;
     plic::curv_cells<<<(int)(need < full ? need : full), plic::kCurvBlock, 0, stream>>>(

@@ -145,6 +145,18 @@ def test_shapes_borders_capacity_empty(plic):
     assert work[0] == work_full[0] > 100
     done = part != 0
     assert 0 < done.sum() <= 100 and np.array_equal(part[done], full[done])
+    # odd cell count (scalar trailing cells of the vector kernel) and a lattice off the 16-byte
+    # boundary (scalar kernel): same result as the oracle / as the aligned call, bit for bit
+    phi = lattices.sphere((13, 15, 17), (8.4, 7.3, 6.6), 4.5)
+    assert phi.size % 4 == 3
+    check(plic, phi, "odd shape", 100)
+    aligned, _ = run_gpu(plic, phi)
+    buf = torch.zeros(phi.size + 1, device="cuda")
+    view = buf[1:].view(phi.shape)
+    view.copy_(torch.from_numpy(phi))
+    assert view.data_ptr() % 16 == 4
+    out = plic.plic_curvature(view)
+    assert np.array_equal(out.cpu().numpy(), aligned)
     # empty lattice
     t = torch.zeros((0, 4, 4), device="cuda")
     assert plic.plic_curvature(t).shape == (0, 4, 4)
