@@ -414,6 +414,17 @@ def run_ours(args):
                 "roofline_frac": 8 * phi5.numel() / (ms * 1e-3) / 1e9 / measured_peak()[0],
                 "bytes_per_lattice_cell": 8, "minus_kappa_R_mean": float(kk.mean()),
                 "L1_error_eq50": float((kk - 1.0).abs().mean())}
+        if not args.no_cpu_baseline and world == 1 and rank == 0:
+            # the curvature oracle (numpy fp64 + the bisection oracle) on the same lattice, once
+            from oracle import curvature as ocurv
+            import oracle as _o
+            host_phi = phi5.cpu().numpy()
+            t0 = time.perf_counter()
+            ocurv.curvature_lattice(host_phi)
+            dt = time.perf_counter() - t0
+            curv["cpu_baseline"] = {"value": n_if / dt / 1e6, "unit": "M interface points/s",
+                                    "cores": _o.max_threads(), "kind": "oracle",
+                                    "sample": "the whole 256^3 lattice once (%.1f s)" % dt}
         del phi5, kap5, work5
 
     # ---- end to end through the host-array C ABI: pinned host buffers, copies inside ----------

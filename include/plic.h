@@ -43,9 +43,10 @@ typedef struct CUstream_st *cudaStream_t;
 #define PLIC_NUM_METHODS     4
 #define PLIC_METHOD_BLANK 0x40 /* plic_roundtrip_error only: the "blank run" of eq. (33), d0 = V0 - 1/2
                                   in place of a PLIC solve */
-#define PLIC_FAST        0x100 /* approximate SFU roots/reciprocals/trig and branch-free,
-                                  a-priori case selection; without it: IEEE division and
-                                  square root, CUDA libm cbrt/asin/acos/sin/cos */
+#define PLIC_FAST        0x100 /* approximate SFU roots/reciprocals/trig, branch-free a-priori
+                                  case selection, two cells per packed fp32x2 instruction;
+                                  without it: IEEE division and square root, CUDA libm
+                                  cbrt/asin/acos/sin/cos, branches in the paper's order */
 
 /* ---- error codes (functions return 0 on success, never throw, never print) ---------------- */
 #define PLIC_OK               0
@@ -68,9 +69,10 @@ typedef struct CUstream_st *cudaStream_t;
  *
  * The caller owns all memory.  The call allocates nothing, keeps no per-call state, does
  * not synchronise and returns as soon as the kernels are enqueued.  Pointers need only be
- * 4-byte aligned: when all five share one alignment modulo 16 the body runs on 128-bit
- * loads/stores and at most 3 head + 3 tail cells take a scalar kernel; otherwise the whole
- * range takes the scalar kernel (correct, slower).
+ * 4-byte aligned: when all five share one alignment modulo 16 the body runs on 16-byte
+ * accesses (bulk asynchronous copies into shared memory or 128-bit loads, 128-bit stores)
+ * and at most 3 head + 3 tail cells take a scalar kernel; otherwise the whole range takes
+ * the scalar kernel (correct, slower).  Body and scalar kernels give bitwise equal results.
  *
  * Input domain (paper: V0 in [0,1], |n|_2 = 1).  Outside it: V0 < 0 acts as 0, V0 > 1 as 1;
  * n need not be normalised exactly -- every method is written so that
