@@ -181,25 +181,26 @@ map_tma(const float4 *__restrict__ s, const float4 *__restrict__ nx,
             if (first + k * step < ntiles) issue(first + k * step, k);
     }
     __syncthreads();                                                 // barriers initialised
-    int stage = 0;
+    // the stage loop is unrolled so that every stage's shared-memory addresses are constants
     uint32_t parity = 0;
-    for (int64_t tile = first; tile < ntiles; tile += step) {
-        mbar_wait(&full[stage], parity);
-        const float4 *src = buf + stage * 4 * kBlock;
-        // in a ragged last tile the slots past the end hold stale data of an earlier tile
-        // (or nothing): they are computed and dropped, never stored
-        const float4 v = src[tid], a = src[kBlock + tid], b = src[2 * kBlock + tid],
-                     c = src[3 * kBlock + tid];
-        __syncthreads();                                             // stage fully read
-        if (tid == 0) {
-            const int64_t next = tile + kStages * step;
-            if (next < ntiles) issue(next, stage);
-        }
-        const int64_t i = tile * kBlock + tid;
-        if (i < n4) st_stream(out + i, OP::apply4(v, a, b, c));
-        if (++stage == kStages) {
-            stage = 0;
-            parity ^= 1;
+    for (int64_t tile = first; tile < ntiles; parity ^= 1) {
+#pragma unroll
+        for (int stage = 0; stage < kStages; ++stage) {
+            if (tile >= ntiles) break;
+            mbar_wait(&full[stage], parity);
+            const float4 *src = buf + stage * 4 * kBlock;
+            // in a ragged last tile the slots past the end hold stale data of an earlier tile
+            // (or nothing): they are computed and dropped, never stored
+            const float4 v = src[tid], a = src[kBlock + tid], b = src[2 * kBlock + tid],
+                         c = src[3 * kBlock + tid];
+            __syncthreads();                                         // stage fully read
+            if (tid == 0) {
+                const int64_t next = tile + kStages * step;
+                if (next < ntiles) issue(next, stage);
+            }
+            const int64_t i = tile * kBlock + tid;
+            if (i < n4) st_stream(out + i, OP::apply4(v, a, b, c));
+            tile += step;
         }
     }
 }
