@@ -160,3 +160,15 @@ def test_shapes_borders_capacity_empty(plic):
     # empty lattice
     t = torch.zeros((0, 4, 4), device="cuda")
     assert plic.plic_curvature(t).shape == (0, 4, 4)
+
+
+def test_config5_full_lattice(plic):
+    """configs[4] at full size (256^3, R = 60, phi = fraction of 8^3 sub-cell points inside), in the
+    launch configuration bench.py times: every interface point against the oracle."""
+    import gen
+    phi = gen.sphere_fill_lattice(256, 60.0, (128.3, 127.7, 128.1), 8)
+    g, r, ok = check(plic, phi, "configs[4]", 50000)
+    kk = -g[ok] * 60.0
+    # phi quantised in steps of 1/512 is a noisy interface: the mean is right, the L1 error large
+    assert abs(kk.mean() - 1.0) < 0.03
+    assert abs(np.abs(kk - 1.0).mean() - np.abs(-r[ok] * 60.0 - 1.0).mean()) < 1e-3
