@@ -40,7 +40,12 @@ typedef struct CUstream_st *cudaStream_t;
                                    */
 #define PLIC_METHOD_NESTED   3 /* nested intervals (bisection) for cases (3),(4): sect. 2.5,
                                   Listing 5 */
-#define PLIC_NUM_METHODS     4
+#define PLIC_NUM_METHODS     4 /* the four methods above; each takes PLIC_FAST */
+#define PLIC_METHOD_KAWANO   4 /* the SZ solution as translated from Kawano's Fortran, Listing 3
+                                  (PAPER.md:187-217), kept for the paper's five-way comparison
+                                  and to reproduce its defect: NaN for n = (1,0,0), V0 in {0,1}
+                                  (PAPER.md:217, 256).  Not edge-case complete, not accurate for
+                                  small normal components; no PLIC_FAST form.  Use PLIC_METHOD_SZ. */
 #define PLIC_METHOD_BLANK 0x40 /* plic_roundtrip_error only: the "blank run" of eq. (33), d0 = V0 - 1/2
                                   in place of a PLIC solve */
 #define PLIC_FAST        0x100 /* approximate SFU roots/reciprocals/trig, branch-free a-priori
@@ -78,7 +83,9 @@ typedef struct CUstream_st *cudaStream_t;
  * n need not be normalised exactly -- every method is written so that
  * d0(V0, c n) = c d0(V0, n) up to rounding; n = (0,0,0) gives d0 = 0.  For every finite
  * input the result is finite (no NaN), including n1 = 0, n1 = n2 = 0 and V0 in {0, 1/2, 1}
- * (PAPER.md:155-181, 217).  A NaN input gives an unspecified finite or NaN output.
+ * -- except with PLIC_METHOD_KAWANO, whose NaN at n = (+-1,0,0) (and
+ * permutations), V0 in {0, 1} is the point of it.  A NaN input gives an unspecified finite or
+ * NaN output.
  *
  * Returns PLIC_OK or a negative PLIC_ERR_*.
  */
@@ -179,7 +186,8 @@ int plic_volume_host(const float *d0, const float *nx, const float *ny, const fl
 /* Frees the host-API workspace and streams of every device; safe to call at any time. */
 void plic_host_release(void);
 
-/* "analytic", "sz", "newton", "nested" (+ "-fast" with PLIC_FAST), "blank"; NULL if unknown.
+/* "analytic", "sz", "newton", "nested" (+ "-fast" with PLIC_FAST), "kawano", "blank"; NULL if
+ * unknown.
  * The string is static storage owned by the library. */
 const char *plic_method_name(int method);
 

@@ -24,7 +24,7 @@ import os
 
 from . import build as _build
 
-__all__ = ["METHODS", "FAST", "BLANK", "method_id", "plic_solve", "plic_volume",
+__all__ = ["METHODS", "FAST", "BLANK", "KAWANO", "method_id", "plic_solve", "plic_volume",
            "plic_roundtrip_error", "plic_sphere_solve", "plic_sphere_volume", "plic_curvature",
            "plic_solve_host",
            "plic_volume_host", "plic_host_release", "plic_method_name", "plic_error_string",
@@ -32,6 +32,7 @@ __all__ = ["METHODS", "FAST", "BLANK", "method_id", "plic_solve", "plic_volume",
            "LIB_PATH"]
 
 METHODS = {"analytic": 0, "sz": 1, "newton": 2, "nested": 3}
+KAWANO = 4              # Listing 3 (Kawano's SZ translation), precise only; see include/plic.h
 FAST = 0x100
 BLANK = 0x40            # plic_roundtrip_error only: the blank run of eq. (33)
 LIB_PATH = _build.LIB
@@ -93,6 +94,10 @@ def method_id(method, fast: bool = False) -> int:
             name, fast = name[:-5], True
         if name == "blank":
             return BLANK
+        if name == "kawano":
+            if fast:
+                raise ValueError("the kawano method has no fast form")
+            return KAWANO
         if name not in METHODS:
             raise ValueError("unknown PLIC method %r" % (method,))
         mid = METHODS[name]

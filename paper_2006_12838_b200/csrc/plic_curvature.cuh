@@ -65,8 +65,8 @@ curv_mark(const float *__restrict__ phi, float *__restrict__ kappa, int nx, int 
     }
 }
 
-// Vector form for 16-byte aligned lattices: four cells per thread and two such groups in flight
-// per thread (32 B loaded before anything is consumed); the ncells % 4 trailing cells are taken
+// Vector form for 16-byte aligned lattices: four cells per float4 group and kMarkGroups groups in
+// flight per thread (64 B loaded before anything is consumed); the ncells % 4 trailing cells are taken
 // by the first threads of block 0.  Same list semantics as curv_mark.
 __device__ __forceinline__ void curv_append(unsigned hits, int64_t first, int *__restrict__ list,
                                             int capacity) {
@@ -92,6 +92,8 @@ __device__ __forceinline__ void curv_append(unsigned hits, int64_t first, int *_
         }
 }
 
+constexpr int kMarkGroups = 4;      // float4 groups per thread per step of curv_mark4
+
 __global__ void __launch_bounds__(256)
 curv_mark4(const float4 *__restrict__ phi, float4 *__restrict__ kappa, int nx, int ny, int nz,
            int *__restrict__ list, int capacity) {
@@ -100,23 +102,28 @@ curv_mark4(const float4 *__restrict__ phi, float4 *__restrict__ kappa, int nx, i
     const int64_t stride = (int64_t)gridDim.x * 256;
     const float4 zero4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     // whole warps iterate together (the append uses warp collectives): bound by the warp's first lane
-    for (int64_t base = (int64_t)blockIdx.x * 256 + (threadIdx.x & ~31); base < n4; base += 2 * stride) {
-        const int64_t g0 = base + (threadIdx.x & 31), g1 = g0 + stride;
-        const bool in0 = g0 < n4, in1 = g1 < n4;
-        float4 p0 = zero4, p1 = zero4;
-        if (in0) p0 = __ldg(phi + g0);
-        if (in1) p1 = __ldg(phi + g1);
-        if (in0) kappa[g0] = zero4;
-        if (in1) kappa[g1] = zero4;
-        const float v0[4] = {p0.x, p0.y, p0.z, p0.w}, v1[4] = {p1.x, p1.y, p1.z, p1.w};
-        unsigned h0 = 0, h1 = 0;
+    for (int64_t base = (int64_t)blockIdx.x * 256 + (threadIdx.x & ~31); base < n4;
+         base += kMarkGroups * stride) {
+        int64_t g[kMarkGroups];
+        float4 p[kMarkGroups];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            if (v0[c] > 0.0f && v0[c] < 1.0f && curv_interior(4 * g0 + c, nx, ny, nz)) h0 |= 1u << c;
-            if (v1[c] > 0.0f && v1[c] < 1.0f && curv_interior(4 * g1 + c, nx, ny, nz)) h1 |= 1u << c;
+        for (int k = 0; k < kMarkGroups; ++k) {                      // all loads first
+            g[k] = base + (threadIdx.x & 31) + k * stride;
+            p[k] = zero4;
+            if (g[k] < n4) p[k] = __ldg(phi + g[k]);
         }
-        curv_append(h0, 4 * g0, list, capacity);
-        curv_append(h1, 4 * g1, list, capacity);
+#pragma unroll
+        for (int k = 0; k < kMarkGroups; ++k)
+            if (g[k] < n4) kappa[g[k]] = zero4;
+#pragma unroll
+        for (int k = 0; k < kMarkGroups; ++k) {
+            const float v[4] = {p[k].x, p[k].y, p[k].z, p[k].w};
+            unsigned h = 0;
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+                if (v[c] > 0.0f && v[c] < 1.0f && curv_interior(4 * g[k] + c, nx, ny, nz)) h |= 1u << c;
+            curv_append(h, 4 * g[k], list, capacity);
+        }
     }
     if (blockIdx.x == 0 && threadIdx.x < 32) {                    // the ncells % 4 trailing cells
         const int64_t i = 4 * n4 + threadIdx.x;

@@ -223,7 +223,7 @@ map_scalar(const float *__restrict__ s, const float *__restrict__ nx,
 // ---------------------------------------------------------------------------------------
 // launch geometry: persistent grid = SMs x resident blocks per SM, cached per device/kernel
 // ---------------------------------------------------------------------------------------
-constexpr int kNumKernels = 2 * PLIC_NUM_METHODS + 1;      // 8 solve variants + volume
+constexpr int kNumKernels = 2 * PLIC_NUM_METHODS + 2;      // 8 solve variants + volume + Kawano
 
 struct DeviceInfo {
     std::once_flag once;
@@ -261,6 +261,7 @@ static BodyKernel vec_kernel(int k) {
         case 5: return body_of<SolveOp<SZ, true>>();
         case 6: return body_of<SolveOp<NEWTON, true>>();
         case 7: return body_of<SolveOp<NESTED, true>>();
+        case 9: return body_of<SolveOp<KAWANO, false>>();
         default: return body_of<VolumeOp>();
     }
 }
@@ -274,12 +275,14 @@ static scalar_kernel_t scalar_kernel(int k) {
         case 5: return map_scalar<SolveOp<SZ, true>>;
         case 6: return map_scalar<SolveOp<NEWTON, true>>;
         case 7: return map_scalar<SolveOp<NESTED, true>>;
+        case 9: return map_scalar<SolveOp<KAWANO, false>>;
         default: return map_scalar<VolumeOp>;
     }
 }
 
 // kernel index for a method id; -1 if the id is unknown
 static int kernel_index(int method) {
+    if (method == PLIC_METHOD_KAWANO) return 2 * PLIC_NUM_METHODS + 1;     // precise only
     const int base = method & ~PLIC_FAST;
     if (base < 0 || base >= PLIC_NUM_METHODS) return -1;
     return base + ((method & PLIC_FAST) ? PLIC_NUM_METHODS : 0);
@@ -395,8 +398,13 @@ roundtrip_kernel(const float *__restrict__ nx, const float *__restrict__ ny,
             // V0_l = l / (L - 1); the last one is exactly 1.  For odd L the second half of the
             // last pair is a repeat of V0 = 1 and is not accumulated.
             const F2 V0{l >= L - 1 ? 1.0f : (float)l * h, l + 1 >= L - 1 ? 1.0f : (float)(l + 1) * h};
-            const F2 V = volume_pair(PairOffset<METHOD, FAST>::d0(V0, X, Y, Z), X, Y, Z);
-            const F2 err = abs2(sub2(V, V0));                                   // eq. (31)
+            const F2 d0 = PairOffset<METHOD, FAST>::d0(V0, X, Y, Z);
+            const F2 V = volume_pair(d0, X, Y, Z);
+            F2 err = abs2(sub2(V, V0));                                         // eq. (31)
+            if (METHOD == KAWANO) {          // Listing 3's NaN propagates into the average;
+                if (d0.x != d0.x) err.x = d0.x;   // volume_pair itself never returns NaN
+                if (d0.y != d0.y) err.y = d0.y;
+            }
             acc.x += err.x;
             if (l + 1 < L) acc.y += err.y;
         }
@@ -416,6 +424,7 @@ static roundtrip_kernel_t roundtrip_kernel_of(int k) {
         case 5: return roundtrip_kernel<SZ, true>;
         case 6: return roundtrip_kernel<NEWTON, true>;
         case 7: return roundtrip_kernel<NESTED, true>;
+        case 9: return roundtrip_kernel<KAWANO, false>;
         default: return roundtrip_kernel<-1, true>;
     }
 }
@@ -629,7 +638,7 @@ int plic_curvature(const float *phi, float *kappa, int nx, int ny, int nz, int32
     if (cudaMemsetAsync(work, 0, sizeof(int32_t), stream) != cudaSuccess) return PLIC_ERR_LAUNCH;
     int64_t need, full = (int64_t)info->sms * 8;
     if ((((uintptr_t)phi | (uintptr_t)kappa) & 15u) == 0 && ncells >= 4) {
-        need = (ncells / 4 + 511) / 512;                             // two float4 groups per thread
+        need = (ncells / 4 + 256 * plic::kMarkGroups - 1) / (256 * plic::kMarkGroups);
         plic::curv_mark4<<<(int)(need < full ? need : full), 256, 0, stream>>>(
             (const float4 *)phi, (float4 *)kappa, nx, ny, nz, work, capacity);
     } else {
@@ -674,6 +683,7 @@ const char *plic_method_name(int method) {
         "analytic",      "sz",      "newton",      "nested",
         "analytic-fast", "sz-fast", "newton-fast", "nested-fast"};
     if (method == PLIC_METHOD_BLANK) return "blank";
+    if (method == PLIC_METHOD_KAWANO) return "kawano";
     const int k = plic::kernel_index(method);
     return k < 0 ? nullptr : names[k];
 }

@@ -36,7 +36,7 @@
 
 namespace plic {
 
-enum : int { ANALYTIC = 0, SZ = 1, NEWTON = 2, NESTED = 3 };
+enum : int { ANALYTIC = 0, SZ = 1, NEWTON = 2, NESTED = 3, KAWANO = 4 };
 
 // ---------------------------------------------------------------------------------------
 // shared pieces
@@ -250,6 +250,64 @@ struct Solver<NESTED, false> {
 };
 
 // ---------------------------------------------------------------------------------------
+// method 4: the SZ solution as implemented by Kawano, "translated ... without further
+// optimization" -- Listing 3, kept for the paper's five-way comparison and
+// for its documented defect: for n = (1,0,0) and V0 in {0, 1} it returns NaN (PAPER.md:217,
+// 256), which is why Tables 1-3 show E_avg = -NaN for it.  NOT edge-case complete and NOT
+// cancellation free (its a2, a1, a0 arithmetic loses the digits of a small m1): use SZ.
+//
+// The listing is truncated in PAPER.md; the surviving lines are followed literally (thresholds
+// v1, v1 + (vm2-vm1)/(2 vm3), v3; cases (1), (2), (5) closed forms; a2, a1, a0 of cases (3)/(4);
+// the 4/3 pi constant; return l*copysign(0.5-alpha, V0-0.5)), the lost ones are filled in from
+// the text (R21): vm_i = n_i / l with the L1 norm l, w = V, w6 =
+// 6 vm1 vm2 vm3 w, v1 = vm1^2 / (6 vm2 vm3 + tiny) with tiny = 1e-30 ("a tiny constant to the
+// denominator"), v3 = its cubic form if vm3 < vm12 else vm12 / (2 vm3)
+// with case (5) taken only in the latter situation, and the textbook trigonometric root of alpha^3 + a2 alpha^2 + a1 alpha + a0:
+// p0 = a2^2/9 - a1/3, q0 = (a1 a2 - 3 a0)/6 - a2^3/27, theta = acos(q0 / sqrt(p0^3)) / 3,
+// alpha = 2 sqrt(p0) cos(theta + 4/3 pi) - a2/3.
+// ---------------------------------------------------------------------------------------
+template <>
+struct Solver<KAWANO, false> {
+    static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
+        const float l = (n1 + n2) + n3;
+        const float vm1 = n1 / l, vm2 = n2 / l, vm3 = n3 / l, vm12 = vm1 + vm2;
+        const float w = V;
+        const float w6 = 6.0f * vm1 * vm2 * vm3 * w;
+        const float v1 = vm1 * vm1 / (6.0f * vm2 * vm3 + 1e-30f);
+        float alpha = 0.0f;
+        if (w < v1) {
+            alpha = cbrtf(w6);                                                         // case (1)
+        } else if (w < v1 + 0.5f * (vm2 - vm1) / vm3) {
+            alpha = 0.5f * (vm1 + sqrtf(vm1 * vm1 + 8.0f * vm2 * vm3 * (w - v1)));     // case (2)
+        } else {
+            const float v3 = vm3 < vm12
+                ? (vm3 * vm3 * (3.0f * vm12 - vm3) + vm1 * vm1 * (vm1 - 3.0f * vm3) +
+                   vm2 * vm2 * (vm2 - 3.0f * vm3)) / (6.0f * vm1 * vm2 * vm3)
+                : 0.5f * vm12 / vm3;
+            // case (5) exists only for vm12 <= vm3 (with vm3 < vm12, w >= v3 is case (4))
+            if (vm12 <= vm3 && v3 <= w) alpha = vm3 * w + 0.5f * vm12;
+            if (alpha == 0.0f) {
+                float a0, a1, a2;
+                if (w < v3) {                                                          // case (3)
+                    a2 = -3.0f * vm12;
+                    a1 = 3.0f * (vm1 * vm1 + vm2 * vm2);
+                    a0 = w6 - vm1 * vm1 * vm1 - vm2 * vm2 * vm2;
+                } else {                                                               // case (4)
+                    a2 = -1.5f;
+                    a1 = 1.5f * (vm1 * vm1 + vm2 * vm2 + vm3 * vm3);
+                    a0 = 0.5f * (w6 - vm1 * vm1 * vm1 - vm2 * vm2 * vm2 - vm3 * vm3 * vm3);
+                }
+                const float p0 = a2 * a2 * (1.0f / 9.0f) - a1 * (1.0f / 3.0f);
+                const float q0 = (a1 * a2 - 3.0f * a0) * (1.0f / 6.0f) - a2 * a2 * a2 * (1.0f / 27.0f);
+                const float theta = acosf(q0 / sqrtf(p0 * p0 * p0)) * (1.0f / 3.0f);
+                alpha = 2.0f * sqrtf(p0) * cosf(theta + 4.1887902f) - a2 * (1.0f / 3.0f);   // 4/3 pi
+            }
+        }
+        return alpha * l;
+    }
+};
+
+// ---------------------------------------------------------------------------------------
 // frame: symmetry reduction (eq. (2)-(5)) -> method -> sign restore (eq. (8))
 // ---------------------------------------------------------------------------------------
 template <int METHOD, bool FAST>
@@ -262,7 +320,8 @@ __device__ __forceinline__ float solve_cell(float V0, float nx, float ny, float 
     const float V = fmaxf(fminf(V0, 1.0f - V0), 0.0f);
     float d = Solver<METHOD, FAST>::reduced_offset(n1, n2, n3, V);
     const float hS = 0.5f * ((n1 + n2) + n3);
-    d = fminf(fmaxf(d, 0.0f), hS);                                     // d in [0, S/2]; drops NaN
+    if (METHOD != KAWANO)                                              // Listing 3 has no clamp: its NaN is kept
+        d = fminf(fmaxf(d, 0.0f), hS);                                 // d in [0, S/2]; drops NaN
     const float r = hS - d;
     return V0 > 0.5f ? r : -r;                                         // eq. (8)
 }

@@ -50,7 +50,8 @@ def test_version_and_names(plic):
     assert plic.plic_version() == 100
     assert [plic.plic_method_name(i) for i in range(4)] == ["analytic", "sz", "newton", "nested"]
     assert plic.plic_method_name(2 | plic.FAST) == "newton-fast"
-    assert plic.plic_method_name(4) is None and plic.plic_method_name(-1) is None
+    assert plic.plic_method_name(4) == "kawano" and plic.plic_method_name(4 | plic.FAST) is None
+    assert plic.plic_method_name(5) is None and plic.plic_method_name(-1) is None
     assert plic.plic_method_name(plic.BLANK) == "blank"
     assert plic.plic_error_string(0) == "ok"
     for code in (-1, -2, -3, -4, -5):
@@ -63,8 +64,11 @@ def test_method_id_marshalling(plic):
     assert plic.method_id("nested-fast") == 0x103
     assert plic.method_id(2) == 2
     assert plic.method_id("blank") == 0x40
+    assert plic.method_id("kawano") == 4
     with pytest.raises(ValueError):
-        plic.method_id("kawano")
+        plic.method_id("kawano-fast")
+    with pytest.raises(ValueError):
+        plic.method_id("applic")
 
 
 def test_argument_validation_needs_no_device(plic):
@@ -84,6 +88,7 @@ def test_argument_validation_needs_no_device(plic):
     # unknown method
     assert lib.plic_solve(p, p, p, p, p, 4, 7, None) == -3
     assert lib.plic_solve(p, p, p, p, p, 4, 0x204, None) == -3
+    assert lib.plic_solve(p, p, p, p, p, 4, 0x104, None) == -3               # kawano has no fast form
     assert lib.plic_solve_host(p, p, p, p, p, 4, -1) == -3
     # plic_roundtrip_error: sizes, method (blank allowed here, not in plic_solve), null
     assert lib.plic_roundtrip_error(None, None, None, None, 0, 256, 0, None) == 0

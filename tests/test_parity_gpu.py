@@ -407,3 +407,34 @@ def test_roundtrip_error_empty_and_validation(plic):
     t = torch.ones(4, device="cuda")
     with pytest.raises(plic.PlicError):
         plic.plic_roundtrip_error(t, t, t, 1)
+
+
+# ------------------------------------------------------------------------------------------
+# PLIC_METHOD_KAWANO: Listing 3 as translated from Kawano's Fortran -- the paper's fifth variant
+# ------------------------------------------------------------------------------------------
+def test_kawano_reproduces_the_papers_nan_and_agrees_elsewhere(plic):
+    # (a) the defect the paper reports: n = (1,0,0), V0 in {0, 1} -> NaN,
+    #     which turns E_avg of the benchmark set into NaN (Tables 1-3: "-NaN")
+    V0 = np.array([0.0, 1.0, 0.0, 1.0, 0.0, 1.0], dtype=np.float32)
+    nx = np.array([1, 1, 0, 0, 0, 0], dtype=np.float32)
+    ny = np.array([0, 0, -1, -1, 0, 0], dtype=np.float32)
+    nz = np.array([0, 0, 0, 0, 1, 1], dtype=np.float32)
+    got = plic.plic_solve(*dev(V0, nx, ny, nz), method="kawano").cpu().numpy()
+    assert np.all(np.isnan(got))
+    for m, f in VARIANTS:                                   # every other variant is finite there
+        ok = plic.plic_solve(*dev(V0, nx, ny, nz), method=m, fast=f).cpu().numpy()
+        assert np.max(np.abs(ok - (V0 - 0.5))) <= 2e-7, (m, f)
+    px, py, pz = gen.paper_normals(4096, seed=22)
+    E = plic.plic_roundtrip_error(*dev(px, py, pz), 64, method="kawano").cpu().numpy()
+    assert np.isnan(E[0]) and np.isnan(E.astype(np.float64).mean())
+    # (b) on normals whose smallest component is not small it is the same solution as the others
+    #     ("apart from floating-point errors ... identical results"); the literal
+    #     a2, a1, a0 arithmetic loses digits as m1 -> 0, hence the restriction and the looser bound
+    V0, nx, ny, nz = gen.random_sphere(1 << 18, seed=23)
+    keep = np.minimum(np.minimum(np.abs(nx), np.abs(ny)), np.abs(nz)) > 0.1
+    V0, nx, ny, nz = V0[keep], nx[keep], ny[keep], nz[keep]
+    ref = oracle.solve(V0, nx, ny, nz)
+    got = plic.plic_solve(*dev(V0, nx, ny, nz), method="kawano").cpu().numpy()
+    assert np.all(np.isfinite(got))
+    assert np.max(np.abs(got.astype(np.float64) - ref)) <= 1e-4
+    assert np.median(np.abs(got.astype(np.float64) - ref)) <= 2e-6
