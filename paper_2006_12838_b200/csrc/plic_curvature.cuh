@@ -68,9 +68,21 @@ curv_mark(const float *__restrict__ phi, float *__restrict__ kappa, int nx, int 
 // Vector form for 16-byte aligned lattices: four cells per float4 group and kMarkGroups groups in
 // flight per thread (64 B loaded before anything is consumed); the ncells % 4 trailing cells are taken
 // by the first threads of block 0.  Same list semantics as curv_mark.
-__device__ __forceinline__ void curv_append(unsigned hits, int64_t first, int *__restrict__ list,
-                                            int capacity) {
-    // hits: bit c set = cell first + c is an interior interface point; warp-aggregated append
+// Hits are collected per block in shared memory (warp-aggregated shared atomics) and flushed to the
+// global list with one global atomicAdd per block, so that no warp waits for a global atomic's
+// round trip inside the streaming loop.  A block that overflows its kMarkCap shared slots appends
+// the excess directly to the global list.
+constexpr int kMarkCap = 2048;
+
+struct MarkShared {
+    int count;
+    int base;
+    int cells[kMarkCap];
+};
+
+__device__ __forceinline__ void curv_append(unsigned hits, int64_t first, MarkShared &sh,
+                                            int *__restrict__ list, int capacity) {
+    // hits: bit c set = cell first + c is an interior interface point
     const int lane = threadIdx.x & 31;
     const int mine = __popc(hits);
     if (__ballot_sync(0xffffffffu, mine > 0) == 0) return;
@@ -81,15 +93,29 @@ __device__ __forceinline__ void curv_append(unsigned hits, int64_t first, int *_
         if (lane >= d) scan += v;
     }
     int start = 0;
-    if (lane == 31) start = atomicAdd(list, scan);
+    if (lane == 31) start = atomicAdd(&sh.count, scan);
     start = __shfl_sync(0xffffffffu, start, 31);
     int slot = start + scan - mine;
 #pragma unroll
     for (int c = 0; c < 4; ++c)
         if (hits & (1u << c)) {
-            if (slot < capacity) list[1 + slot] = (int)(first + c);
+            if (slot < kMarkCap) {
+                sh.cells[slot] = (int)(first + c);
+            } else {                                              // shared list full: straight to global
+                const int g = atomicAdd(list, 1);
+                if (g < capacity) list[1 + g] = (int)(first + c);
+            }
             ++slot;
         }
+}
+
+__device__ __forceinline__ void curv_flush(MarkShared &sh, int *__restrict__ list, int capacity) {
+    __syncthreads();
+    const int n = sh.count < kMarkCap ? sh.count : kMarkCap;
+    if (threadIdx.x == 0 && n > 0) sh.base = atomicAdd(list, n);
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += blockDim.x)
+        if (sh.base + i < capacity) list[1 + sh.base + i] = sh.cells[i];
 }
 
 constexpr int kMarkGroups = 4;      // float4 groups per thread per step of curv_mark4
@@ -101,6 +127,9 @@ curv_mark4(const float4 *__restrict__ phi, float4 *__restrict__ kappa, int nx, i
     const int64_t n4 = ncells / 4;
     const int64_t stride = (int64_t)gridDim.x * 256;
     const float4 zero4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    __shared__ MarkShared sh;
+    if (threadIdx.x == 0) sh.count = 0;
+    __syncthreads();
     // whole warps iterate together (the append uses warp collectives): bound by the warp's first lane
     for (int64_t base = (int64_t)blockIdx.x * 256 + (threadIdx.x & ~31); base < n4;
          base += kMarkGroups * stride) {
@@ -122,7 +151,7 @@ curv_mark4(const float4 *__restrict__ phi, float4 *__restrict__ kappa, int nx, i
 #pragma unroll
             for (int c = 0; c < 4; ++c)
                 if (v[c] > 0.0f && v[c] < 1.0f && curv_interior(4 * g[k] + c, nx, ny, nz)) h |= 1u << c;
-            curv_append(h, 4 * g[k], list, capacity);
+            curv_append(h, 4 * g[k], sh, list, capacity);
         }
     }
     if (blockIdx.x == 0 && threadIdx.x < 32) {                    // the ncells % 4 trailing cells
@@ -133,8 +162,9 @@ curv_mark4(const float4 *__restrict__ phi, float4 *__restrict__ kappa, int nx, i
             reinterpret_cast<float *>(kappa)[i] = 0.0f;
             if (p > 0.0f && p < 1.0f && curv_interior(i, nx, ny, nz)) h = 1u;
         }
-        curv_append(h, i, list, capacity);
+        curv_append(h, i, sh, list, capacity);
     }
+    curv_flush(sh, list, capacity);
 }
 
 // ---- steps 1-6 for one point ----------------------------------------------------------------

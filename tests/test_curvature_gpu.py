@@ -134,6 +134,16 @@ def test_shapes_borders_capacity_empty(plic):
     phi = np.full((6, 6, 6), 0.5, dtype=np.float32)
     got, work = run_gpu(plic, phi)
     assert np.all(got == 0) and work[0] == 4 ** 3
+    # every cell an interface point: more hits per block than its shared list holds (overflow path)
+    rng = np.random.Generator(np.random.Philox(key=43))
+    dense = rng.uniform(0.05, 0.95, (40, 40, 40)).astype(np.float32)
+    got, work = run_gpu(plic, dense)
+    assert work[0] == 38 ** 3
+    assert np.array_equal(np.sort(work[1:1 + work[0]]),
+                          np.sort(np.ravel_multi_index(np.argwhere(np.pad(np.ones((38, 38, 38), bool), 1)).T, dense.shape)))
+    ref = oc.curvature_lattice(dense)
+    m = np.isfinite(ref) & (np.abs(ref) < 10)
+    assert np.max(np.abs(got[m] - ref[m])) <= 1e-3        # 26 noisy neighbours each: well conditioned
     # interface cut by the lattice border: border cells stay 0
     phi = lattices.sphere((16, 16, 16), (8, 8, 2.0), 6)
     got, _ = run_gpu(plic, phi)
