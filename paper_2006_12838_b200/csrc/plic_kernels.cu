@@ -446,7 +446,7 @@ struct SphereVolumeOp {
 };
 
 template <class OP>
-__global__ void __launch_bounds__(kBlock)
+__global__ void __launch_bounds__(kBlock, 8)
 map1_vec4(const float4 *__restrict__ in, float4 *__restrict__ out, int64_t n4) {
     const int64_t stride = (int64_t)gridDim.x * kBlock;
     for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < n4; i += stride) {
