@@ -322,6 +322,26 @@ def test_full_size_config2_sampled(plic):
         assert float((back - tV).abs().max()) <= 2e-5                          # eq. (31)
 
 
+def test_full_size_config4_sampled(plic):
+    """configs[3]: N = 2^28 cells (4.3 GB in, 1.1 GB out), half the normals snapped to an axis or a
+    face diagonal, V0 ~ Beta(1/2, 1/2): properties on every cell, the oracle on every 1024th."""
+    N = 1 << 28
+    V0, nx, ny, nz = gen.snapped_beta(N, seed=3)
+    tV, tx, ty, tz = dev(V0, nx, ny, nz)
+    sl = slice(7, None, 1024)
+    ref = oracle.solve(V0[sl], nx[sl], ny[sl], nz[sl])
+    S2 = 0.5 * (tx.abs() + ty.abs() + tz.abs())
+    out = torch.empty_like(tV)
+    for method, fast in (("analytic", True), ("sz", True), ("newton", True), ("nested", True), ("analytic", False)):
+        plic.plic_solve(tV, tx, ty, tz, out=out, method=method, fast=fast)
+        assert bool(torch.isfinite(out).all())
+        assert bool((out.abs() <= S2 * (1 + 1e-6)).all())
+        got = out[sl].cpu().numpy().astype(np.float64)
+        assert np.max(np.abs(got - ref)) <= TOL_D0, (method, fast)
+    back = plic.plic_volume(out, tx, ty, tz)
+    assert float((back - tV).abs().max()) <= 2e-5                              # eq. (31)
+
+
 # ------------------------------------------------------------------------------------------
 # config 5: sphere of radius 60 on a 256^3 lattice
 # ------------------------------------------------------------------------------------------
