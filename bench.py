@@ -394,6 +394,44 @@ def run_ours(args):
     for k, v in methods.items():
         v["roofline_frac"] = v["hbm_gbs_per_gpu"] / peak
 
+    # ---- divergence cost (the purpose of configs[2]): the same cells, 20 % per intersection case,
+    # once interleaved (case = i mod 5: every warp holds all five cases) and once in five contiguous
+    # blocks (every warp holds one case).  The case label is read off the solved offset.
+    diverg = None
+    if not args.no_divergence and N >= (1 << 24):
+        per = min(1 << 22, N // 32)
+        d0 = plic.plic_solve(dV, dx, dy, dz, method="analytic", fast=False)
+        srt, _ = torch.sort(torch.stack([dx.abs(), dy.abs(), dz.abs()]), dim=0)
+        n1, n2, n3 = srt[0], srt[1], srt[2]
+        dd = 0.5 * (n1 + n2 + n3) - d0.abs()
+        case = torch.where(dd >= n1 + n2, 5, torch.where(dd < n1, 1, torch.where(dd <= n2, 2,
+                           torch.where(dd <= n3, 3, 4))))
+        del srt, n1, n2, n3, dd, d0
+        picks = [torch.nonzero(case == c).flatten()[:per] for c in (1, 2, 3, 4, 5)]
+        del case
+        if all(p.numel() == per for p in picks):
+            contiguous = torch.cat(picks)
+            interleaved = torch.stack(picks, dim=1).flatten()
+            diverg = {"cells": 5 * per, "layout": "20 % per case; interleaved (i mod 5) vs five contiguous blocks",
+                      "source": "the first %d cells of each case among the workload's cells" % per,
+                      "l2": "%.0f MB touched per launch vs 126 MB of L2" % (20 * 5 * per / 1e6), "methods": {}}
+            sets = {}
+            for lay, idx in (("interleaved", interleaved), ("contiguous", contiguous)):
+                sets[lay] = [t[idx].contiguous() for t in (dV, dx, dy, dz)]
+            o5 = torch.empty(5 * per, device="cuda")
+            for m, f in variants:
+                name = plic.plic_method_name(plic.method_id(m, f))
+                r = {}
+                for lay in ("interleaved", "contiguous"):
+                    a = sets[lay]
+                    ms, _ = time_launches(lambda: plic.plic_solve(*a, out=o5, method=m, fast=f),
+                                          args.steps, args.warmup, stream)
+                    r[lay + "_ms"] = max_over_ranks(ms) / args.steps
+                r["interleaved_over_contiguous"] = r["interleaved_ms"] / r["contiguous_ms"]
+                diverg["methods"][name] = r
+            del sets, o5, contiguous, interleaved
+        del picks
+
     # ---- curvature on configs[4]: 256^3 lattice, sphere R = 60 (sect. 4; two launches per call) ----
     curv = None
     if not args.no_curvature:
@@ -483,6 +521,8 @@ def run_ours(args):
             line["paper_benchmark"] = paper
         if curv is not None:
             line["curvature"] = curv
+        if diverg is not None:
+            line["divergence"] = diverg
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(host)
         print(json.dumps(line), flush=True)
@@ -505,6 +545,7 @@ def main(argv=None):
     ap.add_argument("--prewarm-ms", type=float, default=300.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-curvature", action="store_true", help="skip the plic_curvature leg")
+    ap.add_argument("--no-divergence", action="store_true", help="skip the case-stratified divergence leg")
     ap.add_argument("--paper-log2n", type=int, default=24,
                     help="normals in the paper-shaped compute-bound leg = 2^k, L = 256 volumes each "
                          "(the paper: k = 26); 0 skips it")
