@@ -23,6 +23,11 @@ plic_roundtrip_error: 2^k normals x L = 256 volumes in series per thread, blank 
 subtracted, ps per PLIC evaluation and E_avg (eq. 32) per method -- compute bound, for
 comparison with the paper's Titan Xp column (context, not the target).
 
+Further objects on the same line (each timed like the headline, none part of `value`):
+"methods" also lists the plane-sphere maps of sect. 3 (8 B per cell); "divergence" times every
+variant on 20 %-per-case cells, interleaved vs contiguous (the purpose of configs[2]); "curvature"
+times plic_curvature on configs[4] (256^3 lattice, sphere R = 60) with the curvature oracle beside it.
+
 --impl reference times the fp64 CPU oracle (oracle/), as it stands, on the host cores.
 """
 from __future__ import annotations
