@@ -390,6 +390,17 @@ def run_ours(args):
             paper["methods"][name] = {"ms": ms, "ps_per_eval": (ms - raw["blank"][0]) * 1e9 / (PN * PL),
                                       "ps_per_eval_incl_blank": ms * 1e9 / (PN * PL),
                                       "E_avg": None if nan else eavg, "E_avg_is_nan": nan}
+        # issue roofline of the compute-bound loop: thread-instructions per (solve + forward map)
+        # evaluation from the committed ncu capture (profiles/r01_ncu_summary.md, 2c) x evaluations/s,
+        # against 148 SMs x 4 schedulers x 32 lanes x the max SM clock
+        ipe = 78.0
+        sm_max = (sampler.sm_max or 1965) * 1e6
+        peak_tis = 148 * 4 * 32 * sm_max / 1e12
+        ach = ipe * PN * PL / (raw["analytic-fast"][0] * 1e-3) / 1e12
+        paper["roofline"] = {"bound": "alu", "kernel": "roundtrip_kernel<analytic, fast>", "achieved": ach,
+                             "peak": peak_tis, "unit": "T thread-instructions/s", "frac": ach / peak_tis,
+                             "thread_instructions_per_evaluation": ipe,
+                             "peak_source": "148 SMs x 4 x 32 lanes x max SM clock (issue port; DESIGN.md 6)"}
         del pn, pE
 
     solve_names = [plic.plic_method_name(plic.method_id(m, f)) for m, f in variants]
