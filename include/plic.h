@@ -194,7 +194,8 @@ const char *plic_method_name(int method);
 /* Static text for a PLIC_ERR_* code (never NULL). */
 const char *plic_error_string(int code);
 
-/* ABI version: 100*major + minor. */
+/* ABI version: 100*major + minor (1.04: + plic_roundtrip_error, plic_sphere_*, plic_curvature,
+ * PLIC_METHOD_KAWANO). */
 int plic_version(void);
 
 /*

@@ -23,7 +23,7 @@
 #include "plic_packed.cuh"
 #include "plic_curvature.cuh"
 
-#define PLIC_VERSION 100
+#define PLIC_VERSION 104
 
 namespace plic {
 

@@ -47,7 +47,7 @@ def test_header_compiles_as_plain_c(tmp_path):
 
 
 def test_version_and_names(plic):
-    assert plic.plic_version() == 100
+    assert plic.plic_version() == 104
     assert [plic.plic_method_name(i) for i in range(4)] == ["analytic", "sz", "newton", "nested"]
     assert plic.plic_method_name(2 | plic.FAST) == "newton-fast"
     assert plic.plic_method_name(4) == "kawano" and plic.plic_method_name(4 | plic.FAST) is None
