@@ -1,15 +1,16 @@
 // plic_kernels.cu -- kernels, launch logic and the C ABI of libplic (include/plic.h).
 //
 // One elementwise pass per call: 16 B read + 4 B written per cell, no reuse, so the kernels
-// are built around HBM streaming over a persistent grid of (SM count x resident blocks)
-// thread blocks striding over the arrays, one float4 (4 cells) per array per thread per
-// step, 128-bit streaming stores.  Two bodies:
-//   map_tma   the HBM-bound PLIC_FAST kernels (analytic, SZ, Newton): the four input tiles of
-//             a step are brought into shared memory by 1-D bulk asynchronous copies
-//             (cp.async.bulk, SASS UBLKCP) signalled on an mbarrier, kStages tiles ahead of
-//             the arithmetic, so the bytes in flight per SM are set by shared memory
-//             (4 blocks x 3 stages x 16 KB) and not by registers x occupancy;
-//   map_vec4  every other kernel (bound by instruction issue): direct 128-bit
+// are built around HBM streaming, one float4 (4 cells) per array per thread per tile of 1024
+// cells, 128-bit streaming stores.  Two bodies:
+//   map_tma   the HBM-bound kernels (analytic, SZ, Newton fast; plic_volume): a block owns two
+//             consecutive tiles and brings their 8 input pieces into shared memory with 1-D bulk
+//             asynchronous copies (cp.async.bulk, SASS UBLKCP) signalled on mbarriers, issued
+//             all at once; one block per two tiles, scheduled by the hardware, 5 resident per
+//             SM, so the bytes in flight per SM (160 KB) are set by shared memory and not by
+//             registers x occupancy, and fast SMs take more blocks;
+//   map_vec4  every other kernel (bound by instruction issue): a persistent grid of (SM count x
+//             resident blocks) blocks striding over the arrays with direct 128-bit
 //             ld.global.nc.L1::no_allocate loads.
 // Not a contraction: no tensor cores.  Each byte is used exactly once by exactly one thread.
 #include <cuda_runtime.h>
@@ -62,10 +63,10 @@ struct SolveOp {
 template <int METHOD>
 struct SolveOp<METHOD, true> {
     // nested intervals is bound by instruction issue and stays on map_vec4 at 6 blocks per SM
-    // (40 registers); the other three are staged through shared memory (map_tma) at 4 blocks
-    // per SM (64 registers, 4 x 48 KB of stages)
+    // (40 registers); the other three are staged through shared memory (map_tma) at 5 blocks
+    // per SM (48 registers, 5 x 32 KB of tiles)
     static constexpr bool kTma = METHOD != NESTED;
-    static constexpr int kMinBlocks = kTma ? 4 : 6;
+    static constexpr int kMinBlocks = kTma ? 5 : 6;
     static __device__ __forceinline__ float apply(float s, float x, float y, float z) {
         return solve_pair_fast<METHOD>(F2{s, s}, F2{x, x}, F2{y, y}, F2{z, z}).x;
     }
@@ -79,7 +80,7 @@ struct SolveOp<METHOD, true> {
 // plic_volume also runs on packed pairs, branch-free, one division per cell (volume_pair).
 struct VolumeOp {
     static constexpr bool kTma = true;
-    static constexpr int kMinBlocks = 4;
+    static constexpr int kMinBlocks = 5;
     static __device__ __forceinline__ float apply(float s, float x, float y, float z) {
         return volume_pair(F2{s, s}, F2{x, x}, F2{y, y}, F2{z, z}).x;
     }
@@ -108,16 +109,21 @@ map_vec4(const float4 *__restrict__ s, const float4 *__restrict__ nx,
 }
 
 // ---------------------------------------------------------------------------------------
-// map_tma: the same map with the input tiles staged through shared memory by the bulk-copy
-// engine.  A tile is kBlock float4 groups (1024 cells) of each of the four arrays = 16 KB;
-// kStages tiles per block are in flight.  Thread 0 arms full[stage] with the byte count and
-// issues four cp.async.bulk; every thread waits on the barrier's phase, copies its float4s
-// to registers, and after a block barrier (all reads of the stage done) thread 0 refills the
-// stage with the tile kStages steps ahead while the block does the arithmetic and stores.
+// map_tma: the same map with the input tiles brought into shared memory by the bulk-copy
+// engine.  A tile is kBlock float4 groups (1024 cells) of each of the four arrays = 16 KB.  A
+// block owns kTiles consecutive tiles: thread 0 arms one mbarrier per tile with the byte
+// count and issues all 4 kTiles cp.async.bulk at once; every thread then waits for tile 0,
+// copies its float4s to registers, computes and stores, then tile 1, ...  There is no stage
+// reuse, hence no block barrier in the loop and no refill logic.  The grid is NOT persistent:
+// one block per kTiles tiles, handed out by the hardware block scheduler, so SMs that see a
+// shorter memory latency simply take more blocks -- a persistent grid-stride version of this
+// kernel (3 stages, refilled) left 9 % of the SM time idle in its tail and was 5-14 % slower
+// (DESIGN.md section 6).  Pipelining across tiles comes from the 5 resident blocks per SM
+// being at different phases: 10 tiles = 160 KB in flight per SM.
 // ---------------------------------------------------------------------------------------
-constexpr int kStages = 3;
+constexpr int kTiles = 2;                                            // tiles per block
 constexpr int kTileBytes = kBlock * 16;                              // one array's tile
-constexpr int kTmaSmem = kStages * 4 * kTileBytes + kStages * 8;     // stages + mbarriers
+constexpr int kTmaSmem = kTiles * 4 * kTileBytes + kTiles * 8;       // tiles + mbarriers
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {
     return (uint32_t)__cvta_generic_to_shared(p);
@@ -157,51 +163,43 @@ map_tma(const float4 *__restrict__ s, const float4 *__restrict__ nx,
         const float4 *__restrict__ ny, const float4 *__restrict__ nz,
         float4 *__restrict__ out, int64_t n4) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float4 *buf = reinterpret_cast<float4 *>(smem_raw);              // [kStages][4][kBlock]
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + kStages * 4 * kTileBytes);
+    float4 *buf = reinterpret_cast<float4 *>(smem_raw);              // [kTiles][4][kBlock]
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + kTiles * 4 * kTileBytes);
     const int tid = threadIdx.x;
     const int64_t ntiles = (n4 + kBlock - 1) / kBlock;
-    const int64_t first = blockIdx.x, step = gridDim.x;
-
-    auto issue = [&](int64_t tile, int stage) {                      // thread 0 only
-        const int64_t base = tile * kBlock;
-        const int64_t rem = n4 - base;
-        const uint32_t bytes = (uint32_t)(rem < kBlock ? rem : kBlock) * 16u;   // ragged last tile
-        float4 *dst = buf + stage * 4 * kBlock;
-        mbar_expect_tx(&full[stage], 4 * bytes);
-        bulk_g2s(dst, s + base, bytes, &full[stage]);
-        bulk_g2s(dst + kBlock, nx + base, bytes, &full[stage]);
-        bulk_g2s(dst + 2 * kBlock, ny + base, bytes, &full[stage]);
-        bulk_g2s(dst + 3 * kBlock, nz + base, bytes, &full[stage]);
-    };
+    const int64_t first = (int64_t)blockIdx.x * kTiles;
     if (tid == 0) {
-        for (int k = 0; k < kStages; ++k) mbar_init(&full[k], 1);
+        for (int k = 0; k < kTiles; ++k) mbar_init(&full[k], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        for (int k = 0; k < kStages; ++k)
-            if (first + k * step < ntiles) issue(first + k * step, k);
+#pragma unroll
+        for (int k = 0; k < kTiles; ++k) {
+            const int64_t tile = first + k;
+            if (tile < ntiles) {
+                const int64_t base = tile * kBlock;
+                const int64_t rem = n4 - base;
+                const uint32_t bytes = (uint32_t)(rem < kBlock ? rem : kBlock) * 16u;   // ragged last tile
+                float4 *dst = buf + k * 4 * kBlock;
+                mbar_expect_tx(&full[k], 4 * bytes);
+                bulk_g2s(dst, s + base, bytes, &full[k]);
+                bulk_g2s(dst + kBlock, nx + base, bytes, &full[k]);
+                bulk_g2s(dst + 2 * kBlock, ny + base, bytes, &full[k]);
+                bulk_g2s(dst + 3 * kBlock, nz + base, bytes, &full[k]);
+            }
+        }
     }
     __syncthreads();                                                 // barriers initialised
-    // the stage loop is unrolled so that every stage's shared-memory addresses are constants
-    uint32_t parity = 0;
-    for (int64_t tile = first; tile < ntiles; parity ^= 1) {
 #pragma unroll
-        for (int stage = 0; stage < kStages; ++stage) {
-            if (tile >= ntiles) break;
-            mbar_wait(&full[stage], parity);
-            const float4 *src = buf + stage * 4 * kBlock;
-            // in a ragged last tile the slots past the end hold stale data of an earlier tile
-            // (or nothing): they are computed and dropped, never stored
-            const float4 v = src[tid], a = src[kBlock + tid], b = src[2 * kBlock + tid],
-                         c = src[3 * kBlock + tid];
-            __syncthreads();                                         // stage fully read
-            if (tid == 0) {
-                const int64_t next = tile + kStages * step;
-                if (next < ntiles) issue(next, stage);
-            }
-            const int64_t i = tile * kBlock + tid;
-            if (i < n4) st_stream(out + i, OP::apply4(v, a, b, c));
-            tile += step;
-        }
+    for (int k = 0; k < kTiles; ++k) {
+        const int64_t tile = first + k;
+        if (tile >= ntiles) break;
+        mbar_wait(&full[k], 0);
+        const float4 *src = buf + k * 4 * kBlock;
+        // in a ragged last tile the slots past the end were never written: they are computed
+        // and dropped, never stored
+        const float4 v = src[tid], a = src[kBlock + tid], b = src[2 * kBlock + tid],
+                     c = src[3 * kBlock + tid];
+        const int64_t i = tile * kBlock + tid;
+        if (i < n4) st_stream(out + i, OP::apply4(v, a, b, c));
     }
 }
 
@@ -315,9 +313,15 @@ static DeviceInfo *device_info(cudaError_t *err) {
     return info->err == cudaSuccess ? info : nullptr;
 }
 
-static int grid_for(const DeviceInfo *info, int k, int64_t n4) {
-    const int64_t full = (int64_t)info->sms * info->blocks_per_sm[k];
+// grid of the body kernel k over n4 float4 groups (or of a scalar kernel over n4 cells, tma = false):
+// map_tma takes one block per kTiles tiles, the others a persistent grid
+static int grid_for(const DeviceInfo *info, int k, int64_t n4, bool tma) {
     const int64_t need = (n4 + kBlock - 1) / kBlock;
+    if (tma) {
+        const int64_t blocks = (need + kTiles - 1) / kTiles;
+        return (int)(blocks < 1 ? 1 : (blocks > 0x7fffffffLL ? 0x7fffffffLL : blocks));
+    }
+    const int64_t full = (int64_t)info->sms * info->blocks_per_sm[k];
     return (int)(need < full ? (need < 1 ? 1 : need) : full);
 }
 
@@ -345,14 +349,15 @@ static int launch_map(int k, const float *s, const float *nx, const float *ny, c
 
     if (n4 > 0) {
         const BodyKernel body = vec_kernel(k);
-        body.fn<<<grid_for(info, k, n4), kBlock, body.smem, stream>>>(
+        if (body.smem > 0 && (n4 + kBlock - 1) / kBlock > (int64_t)kTiles * 0x7fffffffLL) return PLIC_ERR_SIZE;
+        body.fn<<<grid_for(info, k, n4, body.smem > 0), kBlock, body.smem, stream>>>(
             (const float4 *)(s + head), (const float4 *)(nx + head), (const float4 *)(ny + head),
             (const float4 *)(nz + head), (float4 *)(out + head), n4);
         g_launches.fetch_add(1, std::memory_order_relaxed);
     }
     const int64_t rest = head + (N - tail0);
     if (rest > 0) {
-        scalar_kernel(k)<<<grid_for(info, k, rest), kBlock, 0, stream>>>(s, nx, ny, nz, out, head,
+        scalar_kernel(k)<<<grid_for(info, k, rest, false), kBlock, 0, stream>>>(s, nx, ny, nz, out, head,
                                                                       tail0, N);
         g_launches.fetch_add(1, std::memory_order_relaxed);
     }
@@ -710,7 +715,7 @@ int plic_launch_config(int method, int64_t N, int *grid, int *block, int *cells_
     cudaError_t err;
     const plic::DeviceInfo *info = plic::device_info(&err);
     if (!info) return PLIC_ERR_LAUNCH;
-    *grid = plic::grid_for(info, k, N / 4);
+    *grid = plic::grid_for(info, k, N / 4, plic::vec_kernel(k).smem > 0);
     *block = plic::kBlock;
     *cells_per_thread = 4;
     return PLIC_OK;
