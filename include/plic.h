@@ -201,8 +201,8 @@ int plic_version(void);
 /*
  * plic_launch_config -- the launch geometry plic_solve (method >= 0) or plic_volume
  * (method == -1) uses for N cells with 16-byte aligned pointers on the current device:
- * *grid thread blocks of *block threads, each thread handling *cells_per_thread cells per
- * grid-stride step.  For reporting only.  Returns PLIC_OK or an error code.
+ * *grid thread blocks of *block threads, each thread handling *cells_per_thread cells of each
+ * tile its block owns (one or two tiles per block).  For reporting only.  Returns PLIC_OK or an error code.
  */
 int plic_launch_config(int method, int64_t N, int *grid, int *block, int *cells_per_thread);
 

@@ -92,20 +92,24 @@ struct VolumeOp {
     }
 };
 
-// Body: n4 float4 groups (4 cells each), grid-stride.
+// Body: n4 float4 groups (4 cells each), one block per tile of kBlock groups.  Not a persistent
+// grid: with the tiles handed out by the hardware block scheduler the SMs that run faster (shorter
+// memory latency, less divergent data) take more tiles; a grid-stride version of this kernel
+// over SMs x resident blocks was 7-14 % slower (idle tail), 2-16 tiles per block 1-4 % slower.
+constexpr int kVecTiles = 1;
+
 template <class OP>
 __global__ void __launch_bounds__(kBlock, OP::kMinBlocks)
 map_vec4(const float4 *__restrict__ s, const float4 *__restrict__ nx,
          const float4 *__restrict__ ny, const float4 *__restrict__ nz,
          float4 *__restrict__ out, int64_t n4) {
-    const int64_t stride = (int64_t)gridDim.x * kBlock;
-    for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < n4; i += stride) {
-        const float4 v = ld_stream(s + i);
-        const float4 a = ld_stream(nx + i);
-        const float4 b = ld_stream(ny + i);
-        const float4 c = ld_stream(nz + i);
-        st_stream(out + i, OP::apply4(v, a, b, c));
-    }
+    const int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+    if (i >= n4) return;
+    const float4 v = ld_stream(s + i);
+    const float4 a = ld_stream(nx + i);
+    const float4 b = ld_stream(ny + i);
+    const float4 c = ld_stream(nz + i);
+    st_stream(out + i, OP::apply4(v, a, b, c));
 }
 
 // ---------------------------------------------------------------------------------------
@@ -221,12 +225,9 @@ map_scalar(const float *__restrict__ s, const float *__restrict__ nx,
 // ---------------------------------------------------------------------------------------
 // launch geometry: persistent grid = SMs x resident blocks per SM, cached per device/kernel
 // ---------------------------------------------------------------------------------------
-constexpr int kNumKernels = 2 * PLIC_NUM_METHODS + 2;      // 8 solve variants + volume + Kawano
-
 struct DeviceInfo {
     std::once_flag once;
     int sms = 0;
-    int blocks_per_sm[kNumKernels] = {0};
     cudaError_t err = cudaSuccess;
 };
 static DeviceInfo g_dev[kMaxDevices];
@@ -296,34 +297,19 @@ static DeviceInfo *device_info(cudaError_t *err) {
     }
     DeviceInfo *info = &g_dev[dev];
     std::call_once(info->once, [info, dev]() {
-        cudaError_t e2 = cudaDeviceGetAttribute(&info->sms, cudaDevAttrMultiProcessorCount, dev);
-        for (int k = 0; k < kNumKernels && e2 == cudaSuccess; ++k) {
-            const BodyKernel body = vec_kernel(k);
-            if (body.smem > 0)
-                e2 = cudaFuncSetAttribute(body.fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          body.smem);
-            if (e2 == cudaSuccess)
-                e2 = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&info->blocks_per_sm[k], body.fn,
-                                                                   kBlock, body.smem);
-            if (info->blocks_per_sm[k] < 1) info->blocks_per_sm[k] = 1;
-        }
-        info->err = e2;
+        info->err = cudaDeviceGetAttribute(&info->sms, cudaDevAttrMultiProcessorCount, dev);
     });
     *err = info->err;
     return info->err == cudaSuccess ? info : nullptr;
 }
 
-// grid of the body kernel k over n4 float4 groups (or of a scalar kernel over n4 cells, tma = false):
-// map_tma takes one block per kTiles tiles, the others a persistent grid
-static int grid_for(const DeviceInfo *info, int k, int64_t n4, bool tma) {
-    const int64_t need = (n4 + kBlock - 1) / kBlock;
-    if (tma) {
-        const int64_t blocks = (need + kTiles - 1) / kTiles;
-        return (int)(blocks < 1 ? 1 : (blocks > 0x7fffffffLL ? 0x7fffffffLL : blocks));
-    }
-    const int64_t full = (int64_t)info->sms * info->blocks_per_sm[k];
-    return (int)(need < full ? (need < 1 ? 1 : need) : full);
+// blocks for `units` work items (float4 groups or cells) at kBlock per tile and `per` tiles per block
+static int grid_for(int64_t units, int per) {
+    const int64_t tiles = (units + kBlock - 1) / kBlock;
+    const int64_t blocks = (tiles + per - 1) / per;
+    return (int)(blocks < 1 ? 1 : (blocks > 0x7fffffffLL ? 0x7fffffffLL : blocks));
 }
+static_assert(kTmaSmem <= 48 * 1024, "map_tma fits the default dynamic shared memory limit");
 
 static int launch_map(int k, const float *s, const float *nx, const float *ny, const float *nz,
                       float *out, int64_t N, cudaStream_t stream) {
@@ -349,15 +335,16 @@ static int launch_map(int k, const float *s, const float *nx, const float *ny, c
 
     if (n4 > 0) {
         const BodyKernel body = vec_kernel(k);
-        if (body.smem > 0 && (n4 + kBlock - 1) / kBlock > (int64_t)kTiles * 0x7fffffffLL) return PLIC_ERR_SIZE;
-        body.fn<<<grid_for(info, k, n4, body.smem > 0), kBlock, body.smem, stream>>>(
+        const int per = body.smem > 0 ? kTiles : kVecTiles;
+        if ((n4 + kBlock - 1) / kBlock > (int64_t)per * 0x7fffffffLL) return PLIC_ERR_SIZE;
+        body.fn<<<grid_for(n4, per), kBlock, body.smem, stream>>>(
             (const float4 *)(s + head), (const float4 *)(nx + head), (const float4 *)(ny + head),
             (const float4 *)(nz + head), (float4 *)(out + head), n4);
         g_launches.fetch_add(1, std::memory_order_relaxed);
     }
     const int64_t rest = head + (N - tail0);
     if (rest > 0) {
-        scalar_kernel(k)<<<grid_for(info, k, rest, false), kBlock, 0, stream>>>(s, nx, ny, nz, out, head,
+        scalar_kernel(k)<<<grid_for(rest, 1), kBlock, 0, stream>>>(s, nx, ny, nz, out, head,
                                                                       tail0, N);
         g_launches.fetch_add(1, std::memory_order_relaxed);
     }
@@ -453,12 +440,11 @@ struct SphereVolumeOp {
 template <class OP>
 __global__ void __launch_bounds__(kBlock, 8)
 map1_vec4(const float4 *__restrict__ in, float4 *__restrict__ out, int64_t n4) {
-    const int64_t stride = (int64_t)gridDim.x * kBlock;
-    for (int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x; i < n4; i += stride) {
-        const float4 v = ld_stream(in + i);
-        const F2 lo = OP::apply2(F2{v.x, v.y}), hi = OP::apply2(F2{v.z, v.w});
-        st_stream(out + i, make_float4(lo.x, lo.y, hi.x, hi.y));
-    }
+    const int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x;      // one block per tile, as map_vec4
+    if (i >= n4) return;
+    const float4 v = ld_stream(in + i);
+    const F2 lo = OP::apply2(F2{v.x, v.y}), hi = OP::apply2(F2{v.z, v.w});
+    st_stream(out + i, make_float4(lo.x, lo.y, hi.x, hi.y));
 }
 template <class OP>
 __global__ void __launch_bounds__(kBlock)
@@ -490,7 +476,8 @@ static int launch_map1(const float *in, float *out, int64_t N, cudaStream_t stre
     const int64_t full = (int64_t)info->sms * 8;                     // 8 resident blocks of 256
     if (n4 > 0) {
         const int64_t need = (n4 + kBlock - 1) / kBlock;
-        map1_vec4<OP><<<(int)(need < full ? need : full), kBlock, 0, stream>>>(
+        if (need > 0x7fffffffLL) return PLIC_ERR_SIZE;
+        map1_vec4<OP><<<(int)need, kBlock, 0, stream>>>(
             (const float4 *)(in + head), (float4 *)(out + head), n4);
         g_launches.fetch_add(1, std::memory_order_relaxed);
     }
@@ -606,10 +593,9 @@ int plic_roundtrip_error(const float *nx, const float *ny, const float *nz, floa
     cudaError_t err;
     const plic::DeviceInfo *info = plic::device_info(&err);
     if (!info) return PLIC_ERR_LAUNCH;
-    // compute bound: one thread per normal, at most 8 resident blocks per SM
-    const int64_t need = (N + plic::kBlock - 1) / plic::kBlock;
-    const int64_t full = (int64_t)info->sms * 8;
-    plic::roundtrip_kernel_of(k)<<<(int)(need < full ? need : full), plic::kBlock, 0, stream>>>(
+    // compute bound: one thread per normal, one block per 256 normals (hardware block scheduling)
+    (void)info;
+    plic::roundtrip_kernel_of(k)<<<plic::grid_for(N, 1), plic::kBlock, 0, stream>>>(
         nx, ny, nz, E, N, L);
     plic::g_launches.fetch_add(1, std::memory_order_relaxed);
     return cudaGetLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
@@ -715,7 +701,7 @@ int plic_launch_config(int method, int64_t N, int *grid, int *block, int *cells_
     cudaError_t err;
     const plic::DeviceInfo *info = plic::device_info(&err);
     if (!info) return PLIC_ERR_LAUNCH;
-    *grid = plic::grid_for(info, k, N / 4, plic::vec_kernel(k).smem > 0);
+    *grid = plic::grid_for(N / 4, plic::vec_kernel(k).smem > 0 ? plic::kTiles : plic::kVecTiles);
     *block = plic::kBlock;
     *cells_per_thread = 4;
     return PLIC_OK;

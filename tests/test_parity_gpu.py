@@ -312,8 +312,8 @@ def test_full_size_config2_sampled(plic):
     for method, fast in VARIANTS:
         grid, block, cpt = plic.plic_launch_config(method, N, fast)
         assert block == 256 and cpt == 4
-        # persistent kernels: a multiple of the SM count; map_tma: one block per two tiles of 1024 cells
-        assert grid % 148 == 0 or grid == N // 2048
+        # one block per tile of 1024 cells (map_vec4) or per two tiles (map_tma)
+        assert grid in (N // 1024, N // 2048)
         plic.plic_solve(tV, tx, ty, tz, out=out, method=method, fast=fast)
         assert bool(torch.isfinite(out).all())
         assert bool((out.abs() <= S2 * (1 + 1e-6)).all())
