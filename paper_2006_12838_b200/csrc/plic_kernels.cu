@@ -630,7 +630,7 @@ int plic_curvature(const float *phi, float *kappa, int nx, int ny, int nz, int32
     int64_t need, full = (int64_t)info->sms * 8;
     if ((((uintptr_t)phi | (uintptr_t)kappa) & 15u) == 0 && ncells >= 4) {
         need = (ncells / 4 + 256 * plic::kMarkGroups - 1) / (256 * plic::kMarkGroups);
-        plic::curv_mark4<<<(int)(need < full ? need : full), 256, 0, stream>>>(
+        plic::curv_mark4<<<(int)need, 256, 0, stream>>>(
             (const float4 *)phi, (float4 *)kappa, nx, ny, nz, work, capacity);
     } else {
         need = (ncells + 255) / 256;
