@@ -182,3 +182,18 @@ def test_config5_full_lattice(plic):
     # phi quantised in steps of 1/512 is a noisy interface: the mean is right, the L1 error large
     assert abs(kk.mean() - 1.0) < 0.03
     assert abs(np.abs(kk - 1.0).mean() - np.abs(-r[ok] * 60.0 - 1.0).mean()) < 1e-3
+
+
+def test_l1_error_against_radius(plic):
+    """The shape of the paper's validation (sect. 4.3, eq. (50), fig. 5) without the LBM relaxation:
+    spherical drops initialised with the forward map; L1 curvature error over all interface points."""
+    errs = {}
+    for R in (4, 8, 16, 32):
+        L = 2 * R + 8
+        phi = lattices.sphere((L, L, L), (L / 2 + 0.37, L / 2 - 0.21, L / 2 + 0.13), R)
+        got, _ = run_gpu(plic, phi)
+        k = got[got != 0].astype(np.float64)
+        errs[R] = float(np.abs(-k * R - 1.0).sum() / len(k))              # eq. (50) with kappa_theo = 1/R
+        assert abs(float(-k.mean()) * R - 1.0) < 0.03, (R, -k.mean() * R)
+    assert all(e < 0.10 for e in errs.values()), errs
+    assert errs[4] < errs[32]                     # the error grows with R (PAPER.md:402), unrelaxed here
