@@ -31,6 +31,26 @@ def test_cap_of_half_radius_is_5_32():
     assert abs(sphere.sphere_solve(27.0 / 32.0) - R / 2) < 1e-14
 
 
+def _golden_rows():
+    import os
+    rows = []
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "sphere_examples.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                v, d, why = [x.strip() for x in line.split("|", 2)]
+                rows.append((eval(v), eval(d), why))
+    return rows
+
+
+def test_golden_caps():
+    rows = _golden_rows()
+    assert len(rows) >= 7
+    for V0, d_over_r, why in rows:
+        ok = abs(sphere.sphere_solve(V0) - d_over_r * R) < 1e-13 and abs(sphere.sphere_volume(d_over_r * R) - V0) < 1e-14
+        # the row marked "negative control" states a wrong volume on purpose: the oracle must reject it
+        assert ok != ("negative control" in why), (V0, d_over_r, why)
+
+
 def test_closed_form_eq38():
     # eq. (38) exactly as printed, against the bisection
     V = np.concatenate([np.linspace(0.0, 1.0, 4001), 10.0 ** np.linspace(-12, -1, 200),
