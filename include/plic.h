@@ -164,8 +164,8 @@ int plic_sphere_volume(const float *d0, float *V0, int64_t N, cudaStream_t strea
  *
  * Sign: with the normal of eq. (54) pointing out of the fluid, eq. (63) is negative for a convex
  * fluid body (-1/R for a drop of radius R) and positive for a bubble.
- * Two kernels are enqueued on `stream` (a streaming pass and a dense pass over the interface
- * list); errors, ownership and stream semantics as plic_solve.
+ * A 4-byte memset and two kernels are enqueued on `stream` (a streaming pass and, as a programmatic
+ * dependent launch, a dense pass over the interface list); errors, ownership and stream semantics as plic_solve.
  */
 int plic_curvature(const float *phi, float *kappa, int nx, int ny, int nz, int32_t *work,
                    int64_t work_entries, cudaStream_t stream);

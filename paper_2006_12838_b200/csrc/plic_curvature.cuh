@@ -290,6 +290,9 @@ __device__ __forceinline__ float curvature_point(const float (&p)[27]) {
 __global__ void __launch_bounds__(kCurvBlock)
 curv_cells(const float *__restrict__ phi, float *__restrict__ kappa, int nx, int ny,
            const int *__restrict__ list, int capacity) {
+    // launched with programmatic stream serialization: the blocks may become resident while
+    // curv_mark4 drains; nothing of its output is read before this wait
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int found = list[0];
     const int count = found < capacity ? found : capacity;
     const int64_t sy = nx, sz = (int64_t)nx * ny;

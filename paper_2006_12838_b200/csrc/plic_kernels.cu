@@ -639,8 +639,21 @@ int plic_curvature(const float *phi, float *kappa, int nx, int ny, int nz, int32
     }
     need = ((int64_t)capacity + plic::kCurvBlock - 1) / plic::kCurvBlock;
     full = (int64_t)info->sms * 32;
-    plic::curv_cells<<<(int)(need < full ? need : full), plic::kCurvBlock, 0, stream>>>(
-        phi, kappa, nx, ny, work, capacity);
+    {   // programmatic dependent launch: hides the launch latency behind the tail of the marking pass
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(need < full ? need : full));
+        cfg.blockDim = dim3(plic::kCurvBlock);
+        cfg.dynamicSmemBytes = 0;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        const int *list = work;
+        if (cudaLaunchKernelEx(&cfg, plic::curv_cells, phi, kappa, nx, ny, list, capacity) != cudaSuccess)
+            return PLIC_ERR_LAUNCH;
+    }
     plic::g_launches.fetch_add(2, std::memory_order_relaxed);
     return cudaGetLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
 }
