@@ -44,6 +44,15 @@ __device__ __forceinline__ void st_stream(float4 *p, const float4 &v) {
                  : "memory");
 }
 
+// The body kernels are launched with programmatic stream serialization, so that on a stream of
+// back-to-back calls the blocks of the next kernel become resident while the previous one drains
+// and its launch latency is hidden.  Nothing is read from or written to global memory before
+// this wait, which returns once the preceding kernel has completed and its writes are visible
+// (a no-op after anything that is not a kernel).
+__device__ __forceinline__ void grid_dependency_wait() {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 // op(V0-or-d0, nx, ny, nz) -> result, for one cell
 template <int METHOD, bool FAST>
 struct SolveOp {
@@ -103,6 +112,7 @@ __global__ void __launch_bounds__(kBlock, OP::kMinBlocks)
 map_vec4(const float4 *__restrict__ s, const float4 *__restrict__ nx,
          const float4 *__restrict__ ny, const float4 *__restrict__ nz,
          float4 *__restrict__ out, int64_t n4) {
+    grid_dependency_wait();
     const int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x;
     if (i >= n4) return;
     const float4 v = ld_stream(s + i);
@@ -175,6 +185,7 @@ map_tma(const float4 *__restrict__ s, const float4 *__restrict__ nx,
     if (tid == 0) {
         for (int k = 0; k < kTiles; ++k) mbar_init(&full[k], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        grid_dependency_wait();                     // before the first read of global memory
 #pragma unroll
         for (int k = 0; k < kTiles; ++k) {
             const int64_t tile = first + k;
@@ -337,9 +348,20 @@ static int launch_map(int k, const float *s, const float *nx, const float *ny, c
         const BodyKernel body = vec_kernel(k);
         const int per = body.smem > 0 ? kTiles : kVecTiles;
         if ((n4 + kBlock - 1) / kBlock > (int64_t)per * 0x7fffffffLL) return PLIC_ERR_SIZE;
-        body.fn<<<grid_for(n4, per), kBlock, body.smem, stream>>>(
-            (const float4 *)(s + head), (const float4 *)(nx + head), (const float4 *)(ny + head),
-            (const float4 *)(nz + head), (float4 *)(out + head), n4);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)grid_for(n4, per));
+        cfg.blockDim = dim3(kBlock);
+        cfg.dynamicSmemBytes = (size_t)body.smem;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        if (cudaLaunchKernelEx(&cfg, body.fn, (const float4 *)(s + head), (const float4 *)(nx + head),
+                               (const float4 *)(ny + head), (const float4 *)(nz + head),
+                               (float4 *)(out + head), n4) != cudaSuccess)
+            return PLIC_ERR_LAUNCH;
         g_launches.fetch_add(1, std::memory_order_relaxed);
     }
     const int64_t rest = head + (N - tail0);
