@@ -104,3 +104,32 @@ def test_shard_range_partitions_exactly():
                 assert b == c and a <= b
             for lo, hi in spans[:-1]:
                 assert hi % 32 == 0 or hi == N
+
+
+def test_paper_normals_and_roundtrip_volumes():
+    import gen
+    nx, ny, nz = gen.paper_normals(4096, seed=9)
+    assert nx.dtype == np.float32 and nx.shape == (4096,)
+    assert (nx[0], ny[0], nz[0]) == (1.0, 0.0, 0.0)
+    assert abs(nx[1] - np.sqrt(0.5)) < 1e-7 and abs(ny[1] - np.sqrt(0.5)) < 1e-7 and nz[1] == 0.0
+    assert np.all(nz[:512] == 0.0) and np.count_nonzero(nz[512:] == 0.0) == 0    # 12.5 % 2-D normals
+    assert np.max(np.abs(nx.astype(np.float64) ** 2 + ny.astype(np.float64) ** 2 + nz.astype(np.float64) ** 2 - 1)) < 3e-7
+    again = gen.paper_normals(4096, seed=9)
+    assert all(np.array_equal(a, b) for a, b in zip((nx, ny, nz), again))
+    v = gen.roundtrip_volumes(256)
+    assert v.dtype == np.float32 and v[0] == 0.0 and v[-1] == 1.0 and np.all(np.diff(v) > 0)
+    assert np.max(np.abs(v - np.arange(256) / 255.0)) < 1e-7
+    assert gen.roundtrip_volumes(2).tolist() == [0.0, 1.0]
+
+
+def test_sphere_fill_lattice():
+    import gen
+    phi = gen.sphere_fill_lattice(32, 10.0, (16.3, 15.7, 16.1), 8)
+    assert phi.shape == (32, 32, 32) and phi.dtype == np.float32
+    assert phi.min() == 0.0 and phi.max() == 1.0
+    assert abs(phi.sum() - 4.0 / 3.0 * np.pi * 1000.0) < 5.0              # the drop's volume
+    itf = (phi > 0) & (phi < 1)
+    z, y, x = np.nonzero(itf)
+    r = np.sqrt((x + 0.5 - 16.3) ** 2 + (y + 0.5 - 15.7) ** 2 + (z + 0.5 - 16.1) ** 2)
+    assert np.all(np.abs(r - 10.0) <= 0.5 * np.sqrt(3.0) + 1e-9)         # interface cells straddle the sphere
+    assert np.all(np.round(phi[itf] * 512) == phi[itf] * 512)            # fractions of 8^3 points
