@@ -460,3 +460,38 @@ def test_kawano_reproduces_the_papers_nan_and_agrees_elsewhere(plic):
     assert np.all(np.isfinite(got))
     assert np.max(np.abs(got.astype(np.float64) - ref)) <= 1e-4
     assert np.median(np.abs(got.astype(np.float64) - ref)) <= 2e-6
+
+
+# ------------------------------------------------------------------------------------------
+# adversarial normal / volume distributions (none of BASELINE.json's configs, all in the domain)
+# ------------------------------------------------------------------------------------------
+def test_adversarial_distributions(plic):
+    rng = np.random.Generator(np.random.Philox(key=51))
+    N = 1 << 19
+
+    def unit(g):
+        return g / np.linalg.norm(g, axis=1)[:, None]
+
+    sets = {}
+    g = rng.standard_normal((N, 3)); g[:, 0] *= 10.0 ** rng.uniform(-12, 0, N)
+    sets["tiny n1"] = (unit(g), rng.random(N))
+    g = rng.standard_normal((N, 3)); g[:, 0] *= 10.0 ** rng.uniform(-8, 0, N); g[:, 1] *= 10.0 ** rng.uniform(-8, 0, N)
+    sets["tiny n1, n2"] = (unit(g), rng.random(N))
+    g = np.abs(rng.standard_normal((N, 3))); g[:, 1] = g[:, 0] * (1 + rng.uniform(-1e-6, 1e-6, N))
+    sets["n1 ~ n2"] = (unit(g), rng.random(N))
+    g = np.ones((N, 3)) + rng.uniform(-1e-5, 1e-5, (N, 3))
+    sets["n1 ~ n2 ~ n3"] = (unit(g), rng.random(N))
+    third = N // 3
+    sets["V0 near 0, 1, 1/2"] = (unit(rng.standard_normal((N, 3))), np.concatenate([
+        10.0 ** rng.uniform(-12, -2, third), 1 - 10.0 ** rng.uniform(-7, -2, third),
+        0.5 + rng.uniform(-1e-5, 1e-5, N - 2 * third)]))
+    for name, (n, V) in sets.items():
+        n = n[:, rng.permutation(3)] * rng.choice([-1.0, 1.0], (N, 3))
+        V0 = V.astype(np.float32)
+        nx, ny, nz = [np.ascontiguousarray(n[:, i].astype(np.float32)) for i in range(3)]
+        ref = oracle.solve(V0, nx, ny, nz)
+        for method, fast in VARIANTS:
+            check_solve(plic, V0, nx, ny, nz, method, fast, ref=ref, what="%s / %s" % (name, method))
+        d0 = (ref * rng.uniform(0.0, 1.0, N)).astype(np.float32)
+        got = plic.plic_volume(*dev(d0, nx, ny, nz)).cpu().numpy().astype(np.float64)
+        assert np.max(np.abs(got - oracle.volume(d0, nx, ny, nz))) <= TOL_VOL, name
