@@ -23,6 +23,10 @@ plic_roundtrip_error: 2^k normals x L = 256 volumes in series per thread, blank 
 subtracted, ps per PLIC evaluation and E_avg (eq. 32) per method -- compute bound, for
 comparison with the paper's Titan Xp column (context, not the target).
 
+`value` is taken in the sustained regime (300 ms of load before the first timed region; on this pool
+a software power cap then holds the SM clocks at 1.5-1.85 GHz); "burst" repeats the headline variant
+after 0.5 s of idle, at full clocks -- the regime MEASURED_PEAKS.json's copy bandwidth was taken in.
+
 Further objects on the same line (each timed like the headline, none part of `value`):
 "methods" also lists the plane-sphere maps of sect. 3 (8 B per cell); "divergence" times every
 variant on 20 %-per-case cells, interleaved vs contiguous (the purpose of configs[2]); "curvature"
@@ -483,6 +487,21 @@ def run_ours(args):
                                     "sample": "the whole 256^3 lattice once (%.1f s)" % dt}
         del phi5, kap5, work5
 
+    # ---- the headline variant once more after an idle gap: the clocks recover from the power cap,
+    # which is the regime MEASURED_PEAKS.json's burst figure was taken in (reported beside `value`,
+    # which stays the sustained number)
+    hm0, hf0 = (head[:-5], True) if head.endswith("-fast") else (head, False)
+    torch.cuda.synchronize()
+    time.sleep(0.5)
+    bsteps = max(1, min(args.steps, 30))
+    ms, bwin = time_launches(lambda: plic.plic_solve(dV, dx, dy, dz, out=out, method=hm0, fast=hf0),
+                             bsteps, args.warmup, stream)
+    ms = max_over_ranks(ms) / bsteps
+    burst = {"method": head, "steps": bsteps, "ms_per_step": ms, "value": N * world / (ms * 1e-3) / 1e9,
+             "unit": UNIT, "hbm_gbs_per_gpu": BYTES_PER_CELL * N / (ms * 1e-3) / 1e9,
+             "roofline_frac": BYTES_PER_CELL * N / (ms * 1e-3) / 1e9 / peak,
+             "note": "same kernel, timed after 0.5 s of idle (no sustained load before it)"}
+
     # ---- end to end through the host-array C ABI: pinned host buffers, copies inside ----------
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     pin = [torch.from_numpy(a).pin_memory() for a in host]
@@ -536,6 +555,8 @@ def run_ours(args):
                                       "(DESIGN.md section 6), so frac can exceed 1"},
             "methods": methods,
         }
+        burst["clocks"] = sampler.summary([bwin])
+        line["burst"] = burst
         if paper is not None:
             line["paper_benchmark"] = paper
         if curv is not None:
