@@ -2,16 +2,19 @@
 //
 // One elementwise pass per call: 16 B read + 4 B written per cell, no reuse, so the kernels
 // are built around HBM streaming, one float4 (4 cells) per array per thread per tile of 1024
-// cells, 128-bit streaming stores.  Two bodies:
-//   map_tma   the HBM-bound kernels (analytic, SZ, Newton fast; plic_volume): a block owns two
-//             consecutive tiles and brings their 8 input pieces into shared memory with 1-D bulk
-//             asynchronous copies (cp.async.bulk, SASS UBLKCP) signalled on mbarriers, issued
-//             all at once; one block per two tiles, scheduled by the hardware, 5 resident per
-//             SM, so the bytes in flight per SM (160 KB) are set by shared memory and not by
-//             registers x occupancy, and fast SMs take more blocks;
-//   map_vec4  every other kernel (bound by instruction issue): a persistent grid of (SM count x
-//             resident blocks) blocks striding over the arrays with direct 128-bit
-//             ld.global.nc.L1::no_allocate loads.
+// cells, 128-bit streaming stores.  None of the grids is persistent: one block per tile (or two),
+// handed out by the hardware block scheduler ("Launch").  Three bodies:
+//   map_tma      the HBM-bound kernels (analytic, SZ, Newton fast; plic_volume): a block owns two
+//                consecutive tiles and brings their 8 input pieces into shared memory with 1-D bulk
+//                asynchronous copies (cp.async.bulk, SASS UBLKCP) signalled on mbarriers, issued
+//                all at once; 5 blocks resident per SM, so the bytes in flight per SM (160 KB) are
+//                set by shared memory and not by registers x occupancy;
+//   map_vec4     kernels bound by instruction issue (nested-fast, kawano): direct 128-bit
+//                ld.global.nc.L1::no_allocate loads, one block per tile;
+//   map_compact  the four precise methods (IEEE roots, libm trig, the paper's case order): every
+//                cell takes the branch-free cheap part, the cells of the expensive cases (3)/(4)
+//                and (1) are collected per tile in shared memory and evaluated by dense warps, so
+//                that a warp never runs a case for a handful of its lanes.
 // Not a contraction: no tensor cores.  Each byte is used exactly once by exactly one thread.
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -38,6 +41,15 @@ __device__ __forceinline__ float4 ld_stream(const float4 *p) {
                  : "l"(p));
     return v;
 }
+// the first input may be the output array (in-place call): no .nc on it
+__device__ __forceinline__ float4 ld_stream_rw(const float4 *p) {
+    float4 v;
+    asm volatile("ld.global.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                 : "l"(p)
+                 : "memory");
+    return v;
+}
 __device__ __forceinline__ void st_stream(float4 *p, const float4 &v) {
     asm volatile("st.global.cs.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(v.x), "f"(v.y),
                  "f"(v.z), "f"(v.w)
@@ -54,10 +66,14 @@ __device__ __forceinline__ void grid_dependency_wait() {
 }
 
 // op(V0-or-d0, nx, ny, nz) -> result, for one cell
+enum : int { BODY_VEC4 = 0, BODY_TMA = 1, BODY_COMPACT = 2 };
+
 template <int METHOD, bool FAST>
 struct SolveOp {
     static constexpr int kMinBlocks = 0;      // resident blocks per SM asked of ptxas; 0 = its choice
-    static constexpr bool kTma = false;       // body kernel: map_vec4
+    // the four precise methods run on map_compact, Listing 3 (kawano) on map_vec4
+    static constexpr int kBody = METHOD == KAWANO ? BODY_VEC4 : BODY_COMPACT;
+    static constexpr int kMethod = METHOD;
     static __device__ __forceinline__ float apply(float s, float x, float y, float z) {
         return solve_cell<METHOD, FAST>(s, x, y, z);
     }
@@ -74,8 +90,8 @@ struct SolveOp<METHOD, true> {
     // nested intervals is bound by instruction issue and stays on map_vec4 at 6 blocks per SM
     // (40 registers); the other three are staged through shared memory (map_tma) at 5 blocks
     // per SM (48 registers, 5 x 32 KB of tiles)
-    static constexpr bool kTma = METHOD != NESTED;
-    static constexpr int kMinBlocks = kTma ? 5 : 6;
+    static constexpr int kBody = METHOD != NESTED ? BODY_TMA : BODY_VEC4;
+    static constexpr int kMinBlocks = kBody == BODY_TMA ? 5 : 6;
     static __device__ __forceinline__ float apply(float s, float x, float y, float z) {
         return solve_pair_fast<METHOD>(F2{s, s}, F2{x, x}, F2{y, y}, F2{z, z}).x;
     }
@@ -88,7 +104,7 @@ struct SolveOp<METHOD, true> {
 };
 // plic_volume also runs on packed pairs, branch-free, one division per cell (volume_pair).
 struct VolumeOp {
-    static constexpr bool kTma = true;
+    static constexpr int kBody = BODY_TMA;
     static constexpr int kMinBlocks = 5;
     static __device__ __forceinline__ float apply(float s, float x, float y, float z) {
         return volume_pair(F2{s, s}, F2{x, x}, F2{y, y}, F2{z, z}).x;
@@ -109,13 +125,13 @@ constexpr int kVecTiles = 1;
 
 template <class OP>
 __global__ void __launch_bounds__(kBlock, OP::kMinBlocks)
-map_vec4(const float4 *__restrict__ s, const float4 *__restrict__ nx,
-         const float4 *__restrict__ ny, const float4 *__restrict__ nz,
-         float4 *__restrict__ out, int64_t n4) {
+map_vec4(const float4 *s, const float4 *__restrict__ nx, const float4 *__restrict__ ny,
+         const float4 *__restrict__ nz, float4 *out, int64_t n4) {
+    // s and out may be the same array (in-place call): no __restrict__, no .nc load on them
     grid_dependency_wait();
     const int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x;
     if (i >= n4) return;
-    const float4 v = ld_stream(s + i);
+    const float4 v = ld_stream_rw(s + i);
     const float4 a = ld_stream(nx + i);
     const float4 b = ld_stream(ny + i);
     const float4 c = ld_stream(nz + i);
@@ -173,9 +189,8 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 
 template <class OP>
 __global__ void __launch_bounds__(kBlock, OP::kMinBlocks)
-map_tma(const float4 *__restrict__ s, const float4 *__restrict__ nx,
-        const float4 *__restrict__ ny, const float4 *__restrict__ nz,
-        float4 *__restrict__ out, int64_t n4) {
+map_tma(const float4 *s, const float4 *__restrict__ nx, const float4 *__restrict__ ny,
+        const float4 *__restrict__ nz, float4 *out, int64_t n4) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float4 *buf = reinterpret_cast<float4 *>(smem_raw);              // [kTiles][4][kBlock]
     uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + kTiles * 4 * kTileBytes);
@@ -218,13 +233,109 @@ map_tma(const float4 *__restrict__ s, const float4 *__restrict__ nx,
     }
 }
 
+// ---------------------------------------------------------------------------------------
+// map_compact: the precise methods with the expensive cases compacted per tile.
+//
+// The precise methods keep IEEE roots and libm cbrt / asin / sin / acos / cos, whose cost
+// (60-110 instructions) is only due for the cells of cases (3)/(4) (38 % of random cells) and
+// (1) (6 %).  With a branch per cell a warp pays for every case any of its lanes is in: 10-15
+// of 32 lanes were active per issued instruction and the kernels ran 1.7-2.4x slower on mixed
+// than on case-sorted cells.  Here a block of 256 threads owns one tile of 1024 cells:
+//   phase 1  every thread reduces its 4 cells (eq. (2)-(5)), evaluates Precise<M>::cheap() --
+//            cases (5) and (2) and the case decision, no branch -- writes the 4 offsets to
+//            `dres`, the reduced cells (n1, n2, n3, V) to `cells`, and appends the slots of its
+//            heavy cells to a queue in shared memory: cases (3)/(4) from the front, case (1)
+//            from the back (one packed shared atomic per warp after a warp scan of the packed
+//            counts);
+//   phase 2  the queue is evaluated by whole warps: entry j by thread j mod 256, the case-(1)
+//            entries starting at a warp boundary, so every warp runs one case with all its
+//            lanes (but the last of each kind), and the results overwrite their `dres` slots;
+//   phase 3  every thread reads its 4 offsets back, restores the sign (eq. (8)) and stores.
+// The arithmetic per cell is that of Solver<M, false>::reduced_offset(), bitwise.
+// ---------------------------------------------------------------------------------------
+constexpr int kTileCells = 4 * kBlock;
+
+template <int METHOD>
+__global__ void __launch_bounds__(kBlock, 5)
+map_compact(const float4 *s, const float4 *__restrict__ nx, const float4 *__restrict__ ny,
+            const float4 *__restrict__ nz, float4 *out, int64_t n4) {
+    __shared__ float4 cells[kTileCells];             // (n1, n2, n3, V) of every cell of the tile
+    __shared__ __align__(16) float dres[kTileCells]; // reduced offset d of every cell of the tile
+    __shared__ unsigned short queue[kTileCells];     // cell slots: heavy-A from the front, heavy-B from the back
+    __shared__ unsigned count;                       // heavy-A entries | heavy-B entries << 16
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    if (tid == 0) count = 0;
+    __syncthreads();
+    grid_dependency_wait();
+    const int64_t i = (int64_t)blockIdx.x * kBlock + tid;
+    const bool live = i < n4;
+    // threads past the end carry the zero normal: case (5), nothing queued
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f), a = v, b = v, c = v;
+    if (live) {
+        v = ld_stream_rw(s + i);
+        a = ld_stream(nx + i);
+        b = ld_stream(ny + i);
+        c = ld_stream(nz + i);
+    }
+    const float V0[4] = {v.x, v.y, v.z, v.w};
+    const float X[4] = {a.x, a.y, a.z, a.w}, Y[4] = {b.x, b.y, b.z, b.w}, Z[4] = {c.x, c.y, c.z, c.w};
+    float d[4], hS[4];
+    int kind[4];
+    unsigned mine = 0;                               // packed counts of this thread
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const Reduced cell = reduce_cell(V0[k], X[k], Y[k], Z[k]);
+        hS[k] = half_l1(cell);
+        d[k] = Precise<METHOD>::cheap(cell.n1, cell.n2, cell.n3, cell.V, kind[k]);
+        mine += (unsigned)kind[k];
+        cells[4 * tid + k] = make_float4(cell.n1, cell.n2, cell.n3, cell.V);
+    }
+    reinterpret_cast<float4 *>(dres)[tid] = make_float4(d[0], d[1], d[2], d[3]);
+    unsigned scan = mine;                            // inclusive warp scan of both counts at once
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1)                 // the shuffle's predicate is "source lane in range"
+        asm("{ .reg .pred p; .reg .u32 t; shfl.sync.up.b32 t|p, %0, %1, 0, 0xffffffff; @p add.u32 %0, %0, t; }"
+            : "+r"(scan)
+            : "r"(o));
+    unsigned pos = 0;
+    if (lane == 31) pos = atomicAdd(&count, scan);
+    pos = __shfl_sync(0xffffffffu, pos, 31) + scan - mine;       // packed queue positions of this thread
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const unsigned idx = kind[k] == KIND_HEAVY_A ? (pos & 0xffffu) : (unsigned)(kTileCells - 1) - (pos >> 16);
+        if (kind[k] != KIND_DONE) queue[idx] = (unsigned short)(4 * tid + k);
+        pos += (unsigned)kind[k];
+    }
+    __syncthreads();
+    const unsigned na = count & 0xffffu, nb = count >> 16;
+    const unsigned na32 = (na + 31u) & ~31u;         // case-(1) entries start at a warp boundary
+    for (unsigned j = tid; j < na32 + nb; j += kBlock) {
+        if (j < na32) {
+            if (j < na) {
+                const unsigned slot = queue[j];
+                const float4 e = cells[slot];
+                dres[slot] = Precise<METHOD>::heavy_a(e.x, e.y, e.z, e.w);
+            }
+        } else {
+            const unsigned slot = queue[(unsigned)(kTileCells - 1) - (j - na32)];
+            const float4 e = cells[slot];
+            dres[slot] = Precise<METHOD>::heavy_b(e.x, e.y, e.z, e.w);
+        }
+    }
+    __syncthreads();
+    if (!live) return;
+    const float4 r = reinterpret_cast<const float4 *>(dres)[tid];
+    st_stream(out + i, make_float4(restore_cell<true>(V0[0], hS[0], r.x), restore_cell<true>(V0[1], hS[1], r.y),
+                                   restore_cell<true>(V0[2], hS[2], r.z), restore_cell<true>(V0[3], hS[3], r.w)));
+}
+
 // Scalar: cells [0, head) and [tail0, N) (head/tail of the vector body), or the whole
 // range when the five pointers do not share an alignment (head = N).
 template <class OP>
 __global__ void __launch_bounds__(kBlock)
-map_scalar(const float *__restrict__ s, const float *__restrict__ nx,
-           const float *__restrict__ ny, const float *__restrict__ nz,
-           float *__restrict__ out, int64_t head, int64_t tail0, int64_t N) {
+map_scalar(const float *s, const float *__restrict__ nx, const float *__restrict__ ny,
+           const float *__restrict__ nz, float *out, int64_t head, int64_t tail0, int64_t N) {
     const int64_t stride = (int64_t)gridDim.x * kBlock;
     const int64_t count = head + (N - tail0);
     for (int64_t j = (int64_t)blockIdx.x * kBlock + threadIdx.x; j < count; j += stride) {
@@ -234,7 +345,7 @@ map_scalar(const float *__restrict__ s, const float *__restrict__ nx,
 }
 
 // ---------------------------------------------------------------------------------------
-// launch geometry: persistent grid = SMs x resident blocks per SM, cached per device/kernel
+// launch geometry: one block per tile (map_vec4, map_compact) or per kTiles tiles (map_tma)
 // ---------------------------------------------------------------------------------------
 struct DeviceInfo {
     std::once_flag once;
@@ -249,17 +360,20 @@ typedef void (*vec_kernel_t)(const float4 *, const float4 *, const float4 *, con
 typedef void (*scalar_kernel_t)(const float *, const float *, const float *, const float *,
                                 float *, int64_t, int64_t, int64_t);
 
-// body kernel of an op and the dynamic shared memory it needs
+// body kernel of an op, the dynamic shared memory it needs and the tiles one block takes
 struct BodyKernel {
     vec_kernel_t fn;
     int smem;
+    int tiles;
 };
 template <class OP>
 static BodyKernel body_of() {
-    if constexpr (OP::kTma)
-        return BodyKernel{map_tma<OP>, kTmaSmem};
+    if constexpr (OP::kBody == BODY_TMA)
+        return BodyKernel{map_tma<OP>, kTmaSmem, kTiles};
+    else if constexpr (OP::kBody == BODY_COMPACT)
+        return BodyKernel{map_compact<OP::kMethod>, 0, 1};
     else
-        return BodyKernel{map_vec4<OP>, 0};
+        return BodyKernel{map_vec4<OP>, 0, kVecTiles};
 }
 static BodyKernel vec_kernel(int k) {
     switch (k) {
@@ -346,7 +460,7 @@ static int launch_map(int k, const float *s, const float *nx, const float *ny, c
 
     if (n4 > 0) {
         const BodyKernel body = vec_kernel(k);
-        const int per = body.smem > 0 ? kTiles : kVecTiles;
+        const int per = body.tiles;
         if ((n4 + kBlock - 1) / kBlock > (int64_t)per * 0x7fffffffLL) return PLIC_ERR_SIZE;
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3((unsigned)grid_for(n4, per));
@@ -736,7 +850,7 @@ int plic_launch_config(int method, int64_t N, int *grid, int *block, int *cells_
     cudaError_t err;
     const plic::DeviceInfo *info = plic::device_info(&err);
     if (!info) return PLIC_ERR_LAUNCH;
-    *grid = plic::grid_for(N / 4, plic::vec_kernel(k).smem > 0 ? plic::kTiles : plic::kVecTiles);
+    *grid = plic::grid_for(N / 4, plic::vec_kernel(k).tiles);
     *block = plic::kBlock;
     *cells_per_thread = 4;
     return PLIC_OK;

@@ -66,39 +66,101 @@ __device__ __forceinline__ float cbrt_seed(float k) {
 }
 
 // ---------------------------------------------------------------------------------------
-// method 0: the paper's analytic inverse, eq. (25)/(26), order (5)->(2)->(1)->(3)->(4)
+// The precise methods in three pieces.  A random warp holds all five intersection cases
+// ("GPUs are especially bad at branching"), so each method is split into
+//   cheap()    cases (5) and (2): two closed forms, evaluated for every cell without a branch,
+//              and the case decision `kind` (a priori, eq. (26) with the misprint corrected);
+//   heavy_a()  cases (3)/(4): the expensive root (trigonometric, Newton-Raphson, bisection),
+//              one code path for both cases with (3)/(4) chosen a priori by is_case4();
+//   heavy_b()  case (1): the cube root (libm cbrtf, or Newton-Raphson on d^3 = 6 V n1 n2 n3).
+// The scalar form reduced_offset() branches on `kind` in the paper's order (5)->(2)->(1)->(3)->(4);
+// the streaming body (map_compact in plic_kernels.cu) runs cheap() for all cells, collects the
+// heavy cells of a 1024-cell tile in shared memory and evaluates them in dense warps.  Both
+// call the same three functions, whose results are formed by fmaf / min / max / select or
+// round-to-nearest intrinsics only, so that no multiply is contracted with an add of the caller
+// and the two forms agree bitwise.
 // ---------------------------------------------------------------------------------------
-template <int METHOD, bool FAST>
-struct Solver;
+// `kind` doubles as the increment of map_compact's packed queue counter (heavy-A entries in the
+// low half, heavy-B entries in the high half)
+enum : int { KIND_DONE = 0, KIND_HEAVY_A = 1, KIND_HEAVY_B = 0x10000 };
 
-// Precise: branches in the paper's order, a-posteriori d3 <= n3.
+template <int METHOD>
+struct Precise;
+
+// Cases (5), (2) and the case decision in n-space (analytic, Newton-Raphson, nested intervals).
+struct CheapN {
+    static __device__ __forceinline__ float cheap(float n1, float n2, float n3, float V, int &kind) {
+        const float n12 = n1 + n2;
+        const float W = 2.0f * V * n3;
+        const float x = 3.0f * W * n2;                                     // 6 V n2 n3
+        const float s1 = n1 * n1;
+        const bool c5 = n12 <= W;                                          // (5) eq. (26)
+        const bool c1 = x < s1;                                            // (1)
+        // (2): n1^2 <= 6 V n2 n3 <= n1^2 + 3 n2 (n2 - n1)   [eq. (26), misprint corrected]
+        const bool c2 = x <= fmaf(3.0f * n2, n2 - n1, s1);
+        const float d5 = fmaf(V, n3, 0.5f * n12);
+        const float d2 = fmaf(0.5f, n1, sqrtf(fmaxf(fmaf(W, n2, -s1 * (1.0f / 12.0f)), 0.0f)));
+        kind = c5 ? KIND_DONE : (c1 ? KIND_HEAVY_B : (c2 ? KIND_DONE : KIND_HEAVY_A));
+        return c5 ? d5 : d2;
+    }
+    static __device__ __forceinline__ float k6(float n1, float n2, float n3, float V) {
+        return __fmul_rn(3.0f * (2.0f * V * n3) * n2, n1);                 // 6 V n1 n2 n3
+    }
+};
+
+// depressed cubic of case (3) or (4), chosen a priori: F(tau) = tau^3 - p tau - r on [lo, hi],
+// d = base + tau, d >= floor
+struct Cubic34 {
+    float p, r, lo, hi, base, floor;
+};
+__device__ __forceinline__ Cubic34 cubic34(float n1, float n2, float n3, float V) {
+    const float n12 = n1 + n2;
+    const float W = 2.0f * V * n3;
+    const float q = n1 * n2;
+    const float e = n3 - n12;
+    const float z = n12 - W;
+    const float ee = e * e;
+    const bool c4 = is_case4(q, e, ee, z);
+    const float hS = 0.5f * (n12 + n3);
+    Cubic34 c;
+    c.p = c4 ? 0.75f * fmaf(4.0f, q, -ee) : 6.0f * q;
+    c.r = c4 ? 1.5f * q * (n3 - W) : 3.0f * q * z;
+    c.lo = c4 ? n3 - hS : -n1;
+    c.hi = c4 ? 0.0f : fminf(e, 0.0f);
+    c.base = c4 ? hS : n12;
+    c.floor = c4 ? n3 : n2;
+    return c;
+}
+
+// ---------------------------------------------------------------------------------------
+// method 0: the paper's analytic inverse, eq. (25)/(26)
+//   (3): d = n12 - 2 sqrt(2 q) g(C3), C3 = 3 z / (4 sqrt(2 q))
+//   (4): d = S/2 - sqrt(u)     g(C4), C4 = 6 q (n3 - W) / u^(3/2),   g(C) = sin(asin(C)/3)
+// as one evaluation with A = 2 q or u: IEEE sqrt and division, libm asinf / sinf.  The paper
+// decides (3)-vs-(4) a posteriori by d3 <= n3, which costs case-(4) cells a
+// second trigonometric root; the a-priori test is equivalent (d3 <= n3 <=> F3(e) <= 0).
+// ---------------------------------------------------------------------------------------
 template <>
-struct Solver<ANALYTIC, false> {
-    static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
+struct Precise<ANALYTIC> : CheapN {
+    static __device__ __forceinline__ float heavy_a(float n1, float n2, float n3, float V) {
         typedef Math<false> M;
         const float n12 = n1 + n2;
         const float W = 2.0f * V * n3;
-        if (n12 <= W) return fmaf(V, n3, 0.5f * n12);                      // (5) eq. (26)
-        const float x = 3.0f * W * n2;
-        const float s1 = n1 * n1;
-        if (x >= s1) {
-            // (2): n1^2 <= 6 V n2 n3 <= n1^2 + 3 n2 (n2 - n1)   [eq. (26), misprint corrected]
-            if (x <= fmaf(3.0f * n2, n2 - n1, s1))
-                return fmaf(0.5f, n1, M::sqrt(fmaxf(fmaf(W, n2, -s1 * (1.0f / 12.0f)), 0.0f)));
-        } else {
-            return M::cbrt(x * n1);                                        // (1)
-        }
         const float q = n1 * n2;
-        const float sq = M::sqrt(q + q);
-        const float C3 = 0.75f * M::div(n12 - W, sq);
-        const float d3 = fmaf(-2.0f * sq, M::sin_third_asin(C3), n12);     // (3)
-        if (d3 <= n3) return fmaxf(d3, n2);
         const float e = n3 - n12;
-        const float u = fmaf(4.0f, q, -e * e);
-        const float su = M::sqrt(u);
-        const float C4 = M::div(6.0f * q * (n3 - W), u * su);
-        const float d4 = fmaf(-su, M::sin_third_asin(C4), 0.5f * (n12 + n3));   // (4)
-        return fmaxf(d4, n3);
+        const float z = n12 - W;
+        const float ee = e * e;
+        const bool c4 = is_case4(q, e, ee, z);
+        const float A = c4 ? fmaf(4.0f, q, -ee) : q + q;                   // u or 2 q
+        const float sA = M::sqrt(A);
+        const float num = c4 ? 6.0f * q * (n3 - W) : 0.75f * z;
+        const float C = M::div(num, c4 ? A * sA : sA);
+        const float amp = c4 ? -sA : -2.0f * sA;
+        const float d = fmaf(amp, M::sin_third_asin(C), c4 ? 0.5f * (n12 + n3) : n12);
+        return fmaxf(d, c4 ? n3 : n2);                                     // bracket floor; drops NaN
+    }
+    static __device__ __forceinline__ float heavy_b(float n1, float n2, float n3, float V) {
+        return Math<false>::cbrt(k6(n1, n2, n3, V));                       // (1)
     }
 };
 
@@ -120,47 +182,61 @@ struct Solver<ANALYTIC, false> {
 // ("SZ cancellation").
 // ---------------------------------------------------------------------------------------
 template <>
-struct Solver<SZ, false> {
-    static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
+struct Precise<SZ> {
+    struct L1 {
+        float S, m1, m2, m3;
+    };
+    static __device__ __forceinline__ L1 normalise(float n1, float n2, float n3) {
+        L1 t;
+        t.S = (n1 + n2) + n3;
+        const float inv = Math<false>::div(1.0f, t.S);
+        t.m1 = n1 * inv;
+        t.m2 = n2 * inv;
+        t.m3 = n3 * inv;
+        return t;
+    }
+    static __device__ __forceinline__ float cheap(float n1, float n2, float n3, float V, int &kind) {
+        const L1 t = normalise(n1, n2, n3);
+        const float m12 = t.m1 + t.m2;
+        const float W = 2.0f * V * t.m3;
+        const float x = 3.0f * W * t.m2;                                   // 6 w m2 m3
+        const float s1 = t.m1 * t.m1;                                      // w < v1 <=> x < m1^2
+        const bool c5 = m12 <= W;                                          // (5)
+        const bool c1 = x < s1;                                            // (1)
+        const bool c2 = x <= fmaf(3.0f * t.m2, t.m2 - t.m1, s1);           // (2): v1 <= w <= v2
+        const float a5 = fmaf(V, t.m3, 0.5f * m12);
+        const float a2 = 0.5f * (t.m1 + Math<false>::sqrt(fmaxf(fmaf(4.0f * W, t.m2, -s1 * (1.0f / 3.0f)), 0.0f)));
+        kind = c5 ? KIND_DONE : (c1 ? KIND_HEAVY_B : (c2 ? KIND_DONE : KIND_HEAVY_A));
+        return __fmul_rn(c5 ? a5 : a2, t.S);
+    }
+    static __device__ __forceinline__ float heavy_a(float n1, float n2, float n3, float V) {
         typedef Math<false> M;
-        const float S = (n1 + n2) + n3;
-        const float inv = M::div(1.0f, S);
-        const float m1 = n1 * inv, m2 = n2 * inv, m3 = n3 * inv;
+        const L1 t = normalise(n1, n2, n3);
+        const float m1 = t.m1, m2 = t.m2, m3 = t.m3;
         const float m12 = m1 + m2;
-        const float w = V;
-        const float W = 2.0f * w * m3;
-        float alpha;
-        if (m12 <= W) {
-            alpha = fmaf(w, m3, 0.5f * m12);                                   // (5)
-        } else {
-            const float x = 3.0f * W * m2;                                     // 6 w m2 m3
-            const float s1 = m1 * m1;                                          // w < v1 <=> x < m1^2
-            if (x >= s1 && x <= fmaf(3.0f * m2, m2 - m1, s1)) {                // (2): v1 <= w <= v2
-                alpha = 0.5f * (m1 + M::sqrt(fmaxf(fmaf(4.0f * W, m2, -s1 * (1.0f / 3.0f)), 0.0f)));
-            } else if (x < s1) {
-                alpha = M::cbrt(x * m1);                                       // (1): cbrt(w6)
-            } else {
-                const float q = m1 * m2;
-                bool c4 = false;
-                if (m3 < m12) {
-                    // 6 m1 m2 m3 v3 of Listing 3; case (4) iff w6 >= it
-                    const float s2 = m2 * m2;
-                    float v3n = m3 * m3 * fmaf(3.0f, m12, -m3);
-                    v3n = fmaf(s1, fmaf(-3.0f, m3, m1), v3n);
-                    v3n = fmaf(s2, fmaf(-3.0f, m3, m2), v3n);
-                    c4 = x * m1 >= v3n;
-                }
-                const float em = m12 - m3;
-                const float p0 = c4 ? fmaf(-0.25f * em, em, q) : q + q;
-                const float q0 = c4 ? 0.75f * q * (m3 - W) : 1.5f * q * (m12 - W);
-                const float sp = M::sqrt(p0);
-                const float theta = M::acos(M::div(q0, p0 * sp)) * (1.0f / 3.0f);
-                // cos(theta + 4 pi/3) evaluated as cos(theta - 2 pi/3): same angle, |arg| < pi
-                alpha = fmaf(2.0f * sp, M::cos(theta - 2.0943951f), c4 ? 0.5f : m12);
-                alpha = fmaxf(alpha, c4 ? m3 : m2);                            // bracket floor
-            }
-        }
-        return alpha * S;
+        const float W = 2.0f * V * m3;
+        const float x = 3.0f * W * m2;
+        const float s1 = m1 * m1;
+        const float q = m1 * m2;
+        // 6 m1 m2 m3 v3 of Listing 3; case (4) iff m3 < m12 and w6 >= it
+        float v3n = m3 * m3 * fmaf(3.0f, m12, -m3);
+        v3n = fmaf(s1, fmaf(-3.0f, m3, m1), v3n);
+        v3n = fmaf(m2 * m2, fmaf(-3.0f, m3, m2), v3n);
+        const bool c4 = m3 < m12 && x * m1 >= v3n;
+        const float em = m12 - m3;
+        const float p0 = c4 ? fmaf(-0.25f * em, em, q) : q + q;
+        const float q0 = c4 ? 0.75f * q * (m3 - W) : 1.5f * q * (m12 - W);
+        const float sp = M::sqrt(p0);
+        const float theta = M::acos(M::div(q0, p0 * sp)) * (1.0f / 3.0f);
+        // cos(theta + 4 pi/3) evaluated as cos(theta - 2 pi/3): same angle, |arg| < pi
+        float alpha = fmaf(2.0f * sp, M::cos(theta - 2.0943951f), c4 ? 0.5f : m12);
+        alpha = fmaxf(alpha, c4 ? m3 : m2);                                // bracket floor; drops NaN
+        return __fmul_rn(alpha, t.S);
+    }
+    static __device__ __forceinline__ float heavy_b(float n1, float n2, float n3, float V) {
+        const L1 t = normalise(n1, n2, n3);
+        const float w6 = 3.0f * (2.0f * V * t.m3) * t.m2 * t.m1;
+        return __fmul_rn(Math<false>::cbrt(w6), t.S);                      // (1): cbrt(w6)
     }
 };
 
@@ -171,32 +247,15 @@ struct Solver<SZ, false> {
 // (tau0 = min(0, e) resp. 0), where F is decreasing and concave so the iteration is monotone.
 // ---------------------------------------------------------------------------------------
 template <>
-struct Solver<NEWTON, false> {
-    static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
-        typedef Math<false> M;
-        const float n12 = n1 + n2;
-        const float W = 2.0f * V * n3;
-        if (n12 <= W) return fmaf(V, n3, 0.5f * n12);                      // (5)
-        const float x = 3.0f * W * n2;
-        const float s1 = n1 * n1;
-        if (x >= s1) {
-            if (x <= fmaf(3.0f * n2, n2 - n1, s1))                         // (2)
-                return fmaf(0.5f, n1, M::sqrt(fmaxf(fmaf(W, n2, -s1 * (1.0f / 12.0f)), 0.0f)));
-        } else {
-            const float k = x * n1;                                        // (1)
-            return newton_cubic<false, 3>(0.0f, k, cbrt_seed(k));
-        }
-        const float q = n1 * n2;
-        const float e = n3 - n12;
-        const float z = n12 - W;
-        const float ee = e * e;
-        if (is_case4(q, e, ee, z)) {                                       // (4)
-            const float u = fmaf(4.0f, q, -ee);
-            const float s = newton_cubic<false, 4>(0.75f * u, 1.5f * q * (n3 - W), 0.0f);
-            return fmaxf(0.5f * (n12 + n3) + s, n3);
-        }
-        const float t = newton_cubic<false, 4>(6.0f * q, 3.0f * q * z, fminf(e, 0.0f));   // (3)
-        return fmaxf(n12 + t, n2);
+struct Precise<NEWTON> : CheapN {
+    static __device__ __forceinline__ float heavy_a(float n1, float n2, float n3, float V) {
+        const Cubic34 c = cubic34(n1, n2, n3, V);
+        const float tau = newton_cubic<false, 4>(c.p, c.r, c.hi);
+        return fmaxf(__fadd_rn(c.base, tau), c.floor);
+    }
+    static __device__ __forceinline__ float heavy_b(float n1, float n2, float n3, float V) {
+        const float k = k6(n1, n2, n3, V);                                 // (1)
+        return newton_cubic<false, 3>(0.0f, k, cbrt_seed(k));
     }
 };
 
@@ -217,35 +276,29 @@ __device__ __forceinline__ float bisect_cubic_converged(float p, float r, float 
 }
 
 template <>
-struct Solver<NESTED, false> {
+struct Precise<NESTED> : CheapN {
+    static __device__ __forceinline__ float heavy_a(float n1, float n2, float n3, float V) {
+        const Cubic34 c = cubic34(n1, n2, n3, V);
+        const float tau = bisect_cubic_converged(c.p, c.r, c.lo, c.hi);
+        return fmaxf(__fadd_rn(c.base, tau), c.floor);
+    }
+    static __device__ __forceinline__ float heavy_b(float n1, float n2, float n3, float V) {
+        return Math<false>::cbrt(k6(n1, n2, n3, V));                       // (1)
+    }
+};
+
+template <int METHOD, bool FAST>
+struct Solver;
+
+// scalar form of the four precise methods: branches in the paper's order (5)->(2)->(1)->(3)->(4)
+template <int METHOD>
+struct Solver<METHOD, false> {
     static __device__ __forceinline__ float reduced_offset(float n1, float n2, float n3, float V) {
-        typedef Math<false> M;
-        const float n12 = n1 + n2;
-        const float W = 2.0f * V * n3;
-        const bool c5 = n12 <= W;
-        const float x = 3.0f * W * n2;
-        const float s1 = n1 * n1;
-        float d;
-        if (x < s1) {
-            d = M::cbrt(x * n1);                                               // (1)
-        } else {
-            d = fmaf(0.5f, n1, M::sqrt(fmaxf(fmaf(W, n2, -s1 * (1.0f / 12.0f)), 0.0f)));   // (2)
-        }
-        if (!c5 && x > fmaf(3.0f * n2, n2 - n1, s1)) {
-            const float q = n1 * n2;
-            const float e = n3 - n12;
-            const float z = n12 - W;
-            const float ee = e * e;
-            const bool c4 = is_case4(q, e, ee, z);
-            const float hS = 0.5f * (n12 + n3);
-            const float p = c4 ? 0.75f * fmaf(4.0f, q, -ee) : 6.0f * q;
-            const float r = c4 ? 1.5f * q * (n3 - W) : 3.0f * q * z;
-            const float lo = c4 ? n3 - hS : -n1;
-            const float hi = c4 ? 0.0f : fminf(e, 0.0f);
-            const float tau = bisect_cubic_converged(p, r, lo, hi);
-            d = (c4 ? hS : n12) + tau;
-        }
-        return c5 ? fmaf(V, n3, 0.5f * n12) : d;
+        int kind;
+        float d = Precise<METHOD>::cheap(n1, n2, n3, V, kind);             // (5), (2)
+        if (kind == KIND_HEAVY_B) d = Precise<METHOD>::heavy_b(n1, n2, n3, V);        // (1)
+        else if (kind == KIND_HEAVY_A) d = Precise<METHOD>::heavy_a(n1, n2, n3, V);   // (3), (4)
+        return d;
     }
 };
 
@@ -310,20 +363,33 @@ struct Solver<KAWANO, false> {
 // ---------------------------------------------------------------------------------------
 // frame: symmetry reduction (eq. (2)-(5)) -> method -> sign restore (eq. (8))
 // ---------------------------------------------------------------------------------------
+struct Reduced {
+    float n1, n2, n3, V;
+};
+__device__ __forceinline__ Reduced reduce_cell(float V0, float nx, float ny, float nz) {
+    const float a = fabsf(nx), b = fabsf(ny), c = fabsf(nz);
+    Reduced r;
+    r.n1 = min3(a, b, c);                                              // eq. (2)
+    r.n3 = max3(a, b, c);                                              // eq. (3)
+    r.n2 = fmaxf(fminf(a, b), fminf(fmaxf(a, b), c));                  // eq. (4): the median
+    // eq. (5): 1/2 - |V0 - 1/2| = min(V0, 1 - V0), which is exact in fp32 for V0 in [0,1]
+    r.V = fmaxf(fminf(V0, 1.0f - V0), 0.0f);
+    return r;
+}
+__device__ __forceinline__ float half_l1(const Reduced &c) { return 0.5f * ((c.n1 + c.n2) + c.n3); }   // S/2
+// d0 = sign(V0 - 1/2) (S/2 - d), eq. (8), with d clamped to [0, S/2] (drops a NaN)
+template <bool CLAMP>
+__device__ __forceinline__ float restore_cell(float V0, float hS, float d) {
+    if (CLAMP) d = fminf(fmaxf(d, 0.0f), hS);
+    const float r = __fsub_rn(hS, d);
+    return V0 > 0.5f ? r : -r;
+}
+
 template <int METHOD, bool FAST>
 __device__ __forceinline__ float solve_cell(float V0, float nx, float ny, float nz) {
-    const float a = fabsf(nx), b = fabsf(ny), c = fabsf(nz);
-    const float n1 = min3(a, b, c);                                    // eq. (2)
-    const float n3 = max3(a, b, c);                                    // eq. (3)
-    const float n2 = fmaxf(fminf(a, b), fminf(fmaxf(a, b), c));        // eq. (4): the median
-    // eq. (5): 1/2 - |V0 - 1/2| = min(V0, 1 - V0), which is exact in fp32 for V0 in [0,1]
-    const float V = fmaxf(fminf(V0, 1.0f - V0), 0.0f);
-    float d = Solver<METHOD, FAST>::reduced_offset(n1, n2, n3, V);
-    const float hS = 0.5f * ((n1 + n2) + n3);
-    if (METHOD != KAWANO)                                              // Listing 3 has no clamp: its NaN is kept
-        d = fminf(fmaxf(d, 0.0f), hS);                                 // d in [0, S/2]; drops NaN
-    const float r = hS - d;
-    return V0 > 0.5f ? r : -r;                                         // eq. (8)
+    const Reduced c = reduce_cell(V0, nx, ny, nz);
+    const float d = Solver<METHOD, FAST>::reduced_offset(c.n1, c.n2, c.n3, c.V);
+    return restore_cell<METHOD != KAWANO>(V0, half_l1(c), d);          // Listing 3 has no clamp: its NaN is kept
 }
 
 }  // namespace plic

@@ -115,7 +115,7 @@ __device__ __forceinline__ PairIn pair_reduce(F2 V0, F2 nx, F2 ny, F2 nz) {
     // eq. (5): V = 1/2 - |V0 - 1/2| = min(V0, 1 - V0); the saturation makes V0 < 0 act as 0
     // and V0 > 1 as 1
     const F2 V = min2(V0, fma2(V0, -1.0f, f2(1.0f)));
-    in.V2 = sat2(add2(V, V));
+    in.V2 = F2{__saturatef(V.x + V.x), __saturatef(V.y + V.y)};
     in.n12 = add2(in.n1, in.n2);
     in.hS = mul2(add2(in.n12, in.n3), 0.5f);
     return in;
@@ -157,8 +157,10 @@ struct PairSolver<ANALYTIC> {
         const F2 Wn2 = mul2(W, n2);                                             // x / 3, x = 6 V n2 n3
         const F2 s1 = mul2(n1, n1);
         const F2 t1 = fma2(s1, -1.0f / 3.0f, Wn2);                              // (x - n1^2) / 3
-        // (2) and (1): d1 = cbrt(x n1) = 2^(lg2(Wn2 n1)/3 + lg2(3)/3)
-        const F2 d2 = fma2(n1, 0.5f, sqrt2(max2(fma2(s1, -1.0f / 12.0f, Wn2), 0.0f)));
+        // (2) and (1): d1 = cbrt(x n1) = 2^(lg2(Wn2 n1)/3 + lg2(3)/3).  The radicand of d2 needs no
+        // clamp: where (2) is selected, t1 >= 0, and Wn2 - n1^2/12 >= Wn2 - n1^2/3 = t1 holds for
+        // the rounded FMAs too (monotone in the addend); elsewhere its NaN is dropped by the select
+        const F2 d2 = fma2(n1, 0.5f, sqrt2(fma2(s1, -1.0f / 12.0f, Wn2)));
         const F2 d1 = ex2_2(fma2(lg2_2(mul2(Wn2, n1)), 1.0f / 3.0f, f2(0.528320834f)));
         F2 d = sel2(lt2(t1, f2(0.0f)), d1, d2);                                 // x < n1^2
         // (3)/(4)
@@ -179,14 +181,22 @@ struct PairSolver<ANALYTIC> {
 };
 
 // ---------------------------------------------------------------------------------------
-// method 1, PLIC_FAST: Scardovelli-Zaleski (sect. 2.4) on a pair, branch-free.  Same
-// arithmetic as Solver<SZ, false>, fast roots: L1-normalised m_i = n_i / S, alpha = d / S, thresholds
-// multiplied through, the collapsed p0, q0 (plic_methods.cuh), root
+// method 1, PLIC_FAST: Scardovelli-Zaleski (sect. 2.4) on a pair, branch-free: L1-normalised
+// m_i = n_i / S, alpha = d / S, thresholds multiplied through, (5) and (2) tested first, root
 //   alpha = 2 sqrt(p0) cos(acos(q0 / p0^(3/2)) / 3 + 4 pi / 3) - a2/3
-// with 1/sqrt(p0) from one rsqrt, acos by sqrt(1-x) Q5(x) and cos on the SFU.
+// with the collapsed p0, q0 of Precise<SZ> (plic_methods.cuh).  Micro-optimised further:
+//   * R = 4 p0 (= 8 q in case (3), 4 q - (m3 - m12)^2 in case (4)) and rho = rsqrt(R) give
+//     2 sqrt(p0) = R rho and q0 / p0^(3/2) = 8 q0 rho^3, which in case (3) is (3/2) z rho
+//     (8 q rho^2 = 1) and in case (4) 6 q (m3 - W) rho^3;
+//   * the (3)-vs-(4) threshold w6 >= 6 m1 m2 m3 v3 is the sign of the case-(3)
+//     cubic at alpha = m3, a polynomial in m12 - m3 (is_case4_2), instead of the v3 polynomial;
+//   * the tests (1)/(2)/(3,4) in the scaled variable t1 = W m2 - m1^2 / 3;
+//   * acos by sqrt(1-x) Q5(x), the angle's 1/3 and the 4 pi / 3 in one FMA, cos on the SFU.
+// What distinguishes it from the analytic kernel is the L1 scaling (an SFU reciprocal, four
+// multiplications) and acos + cos in place of the sin(asin(.)/3) polynomial.
 // ---------------------------------------------------------------------------------------
 // acos(x) for x in [0, 1] as sqrt(1-x) * Q5(x), |err| < 1.2e-6 (minimax fit,
-// fit_coefficients.py); the angle is then divided by 3.
+// fit_coefficients.py).
 __device__ __forceinline__ F2 acos_fast2(F2 x) {
     F2 p = fma2(x, f2(-0.004337173733f), f2(0.01934827404f));
     p = fma2(p, x, f2(-0.04495724702f));
@@ -204,32 +214,27 @@ struct PairSolver<SZ> {
         const F2 m1 = mul2(in.n1, inv), m2 = mul2(in.n2, inv), m3 = mul2(in.n3, inv);
         const F2 m12 = add2(m1, m2);
         const F2 W = mul2(in.V2, m3);                                           // 2 w m3
-        const F2 Wm2 = mul2(W, m2);
-        const F2 x = mul2(Wm2, 3.0f);                                           // 6 w m2 m3
+        const F2 Wm2 = mul2(W, m2);                                             // x / 3, x = 6 w m2 m3
         const F2 s1 = mul2(m1, m1);
-        // (2): v1 <= w <= v2, and (1): w < v1  <=>  x < m1^2
-        const F2 a2 = mul2(add2(m1, sqrt2(max2(fma2(s1, -1.0f / 3.0f, mul2(Wm2, 4.0f)), 0.0f))), 0.5f);
-        const F2 a1 = ex2_2(mul2(lg2_2(mul2(x, m1)), 1.0f / 3.0f));             // cbrt(w6)
-        F2 alpha = sel2(lt2(x, s1), a1, a2);
-        // (3)/(4) a priori from v3: case (4) iff m3 < m12 and w6 >= 6 m1 m2 m3 v3
+        const F2 t1 = fma2(s1, -1.0f / 3.0f, Wm2);                              // (x - m1^2) / 3
+        // (2): v1 <= w <= v2, and (1): w < v1  <=>  x < m1^2;  cbrt(w6), w6 = 3 Wm2 m1
+        const F2 a2 = fma2(m1, 0.5f, sqrt2(fma2(s1, -1.0f / 12.0f, Wm2)));
+        const F2 a1 = ex2_2(fma2(lg2_2(mul2(Wm2, m1)), 1.0f / 3.0f, f2(0.528320834f)));
+        F2 alpha = sel2(lt2(t1, f2(0.0f)), a1, a2);
+        // (3)/(4)
         const F2 q = mul2(m1, m2);
-        const F2 m3x3 = mul2(m3, 3.0f);
-        F2 v3n = mul2(mul2(m3, m3), fma2(m12, 3.0f, mul2(m3, -1.0f)));
-        v3n = fma2(s1, sub2(m1, m3x3), v3n);
-        v3n = fma2(mul2(m2, m2), sub2(m2, m3x3), v3n);
-        const F2 w6 = mul2(x, m1);
-        const B2 c4 = B2{m3.x < m12.x && w6.x >= v3n.x, m3.y < m12.y && w6.y >= v3n.y};
-        const F2 em = sub2(m12, m3);
-        const F2 p0 = sel2(c4, fma2(mul2(em, -0.25f), em, q), add2(q, q));
-        const F2 q0 = mul2(q, sel2(c4, mul2(sub2(m3, W), 0.75f), mul2(sub2(m12, W), 1.5f)));
-        const F2 rho = rsqrt2(p0);
-        const F2 arg = mul2(mul2(q0, rho), mul2(rho, rho));                     // q0 / p0^(3/2)
-        const F2 theta = mul2(acos_fast2(min2(arg, f2(1.0f))), 1.0f / 3.0f);
+        const F2 e = sub2(m3, m12);
+        const F2 z = sub2(m12, W);
+        const F2 ee = mul2(e, e);
+        const B2 c4 = is_case4_2(q, e, ee, z);
+        const F2 R = sel2(c4, fma2(q, 4.0f, mul2(ee, -1.0f)), mul2(q, 8.0f));  // 4 p0
+        const F2 rho = rsqrt2(R);
+        const F2 K4 = mul2(mul2(mul2(q, 6.0f), sub2(m3, W)), mul2(rho, rho));
+        const F2 arg = mul2(sel2(c4, K4, mul2(z, 1.5f)), rho);                  // q0 / p0^(3/2)
         // cos(theta + 4 pi/3) evaluated as cos(theta - 2 pi/3): same angle, |arg| < pi
-        const F2 co = cos2(add2(theta, f2(-2.0943951f)));
-        const F2 sp2 = mul2(mul2(p0, rho), 2.0f);                               // 2 sqrt(p0)
-        const F2 a34 = max2(fma2(sp2, co, sel2(c4, f2(0.5f), m12)), m2);        // floor; drops NaN
-        alpha = sel2(gt2(x, fma2(mul2(m2, 3.0f), sub2(m2, m1), s1)), a34, alpha);
+        const F2 co = cos2(fma2(acos_fast2(min2(arg, f2(1.0f))), 1.0f / 3.0f, f2(-2.0943951f)));
+        const F2 a34 = max2(fma2(mul2(R, rho), co, sel2(c4, f2(0.5f), m12)), m2);   // floor; drops NaN
+        alpha = sel2(gt2(t1, mul2(m2, sub2(m2, m1))), a34, alpha);
         alpha = sel2(le2(m12, W), mul2(add2(W, m12), 0.5f), alpha);             // (5)
         return mul2(alpha, S);
     }
@@ -250,7 +255,7 @@ struct PairSolver<NEWTON> {
         const F2 x = mul2(Wn2, 3.0f);
         const F2 s1 = mul2(n1, n1);
         const B2 c1 = lt2(x, s1);
-        const F2 d2 = fma2(n1, 0.5f, sqrt2(max2(fma2(s1, -1.0f / 12.0f, Wn2), 0.0f)));
+        const F2 d2 = fma2(n1, 0.5f, sqrt2(fma2(s1, -1.0f / 12.0f, Wn2)));
         const F2 q = mul2(n1, n2);
         const F2 e = sub2(n3, n12);
         const F2 z = sub2(n12, W);
@@ -258,19 +263,21 @@ struct PairSolver<NEWTON> {
         const B2 c4 = is_case4_2(q, e, ee, z);
         const F2 k = mul2(x, n1);                                               // 6 V n1 n2 n3
         const F2 zero = f2(0.0f);
-        F2 p = sel2(c4, mul2(fma2(q, 4.0f, mul2(ee, -1.0f)), 0.75f), mul2(q, 6.0f));
-        F2 r = mul2(q, sel2(c4, mul2(sub2(n3, W), 1.5f), mul2(z, 3.0f)));
+        // F / 2: the iteration tau <- (tau^3 + r/2) / (3/2 tau^2 - p/2) is the Newton step with
+        // one instruction less (no 2 tau^2); nh = -p/2, rh = r/2
+        F2 nh = sel2(c4, mul2(fma2(q, 4.0f, mul2(ee, -1.0f)), -0.375f), mul2(q, -3.0f));
+        F2 rh = mul2(q, sel2(c4, mul2(sub2(n3, W), 0.75f), mul2(z, 1.5f)));
         F2 tau = sel2(c4, zero, min2(e, zero));
         F2 base = sel2(c4, in.hS, n12);
-        p = sel2(c1, zero, p);
-        r = sel2(c1, k, r);
+        nh = sel2(c1, zero, nh);
+        rh = sel2(c1, mul2(k, 0.5f), rh);
         tau = sel2(c1, F2{cbrt_seed(k.x), cbrt_seed(k.y)}, tau);
         base = sel2(c1, zero, base);
         const F2 floor_ = sel2(c1, zero, n2);
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const F2 t2 = mul2(tau, tau);
-            tau = mul2(fma2(add2(t2, t2), tau, r), rcp2(fma2(t2, 3.0f, mul2(p, -1.0f))));
+            tau = mul2(fma2(t2, tau, rh), rcp2(fma2(t2, 1.5f, nh)));
         }
         const F2 dn = max2(add2(base, tau), floor_);                            // floor; drops NaN
         const F2 thr = fma2(mul2(n2, 3.0f), sub2(n2, n1), s1);
@@ -282,10 +289,49 @@ struct PairSolver<NEWTON> {
 
 // ---------------------------------------------------------------------------------------
 // method 3, PLIC_FAST: nested intervals (sect. 2.5) on a pair: 20 fixed halvings of the
-// bracket of the depressed cubic in branch-free (lo, width) form for (3)/(4) (|err| <= 3e-7;
-// the precise kernel halves until the fp32 midpoint stops moving); closed forms for (1), (2),
-// (5).  F is decreasing on the bracket, F(lo) >= 0.
+// bracket [lo, hi] of the depressed cubic F for (3)/(4) (|err| <= 3.3e-7; the precise kernel
+// halves until the fp32 midpoint stops moving); closed forms for (1), (2), (5).  F is
+// decreasing on the bracket, F(lo) >= 0 >= F(hi).
+//
+// The halving runs in the scaled variable y = tau / (hi - lo), in which the bracket has unit
+// width, and carries the interval's CENTRE c instead of its lower end:
+//     G(y) = y^3 - P y - R,   P = p / w^2,  R = r / w^3,  w = hi - lo      (G = F / w^3)
+//     c_0 = lo/w + 1/2,   c_{k+1} = c_k + copysign(2^-(k+2), G(c_k))
+// G(c) > 0 means the root lies right of c.  The interval after k steps is c_k +- 2^-(k+1), the
+// same sequence of intervals as (lo, hi) bisection.  The step sizes are compile-time
+// constants, so one halving costs two packed FMAs, one sign transfer per half (LOP3:
+// (G & 0x80000000) | 2^-(k+2)) and one packed add -- 5 issued instructions per pair instead of
+// the 8 of the compare-and-select form (FMUL2, FADD2, 2 FFMA2, 2 FSETP, 2 FSEL).  Rounding: c
+// may be large when the bracket is narrow and far from 0 (|lo| >> w), but ulp(c) w = ulp(lo),
+// the resolution tau has anyway.  w = 0 or a flushed product gives NaN or 0, which the floor
+// n2 replaces (the bracket is then narrower than fp32).
 // ---------------------------------------------------------------------------------------
+// The sign mask is read from constant memory so that it sits in a register and the LOP3's one
+// immediate slot is free for the step size (as a literal mask, ptxas moves every step constant
+// into a register first: one more instruction per step).
+__constant__ unsigned kSignMask = 0x80000000u;
+
+template <unsigned STEP_BITS>
+__device__ __forceinline__ float signed_step(float G, unsigned mask) {
+    unsigned r;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(r) : "r"(__float_as_uint(G)), "r"(mask), "n"(STEP_BITS));
+    return __uint_as_float(r);
+}
+
+template <int K, int N>
+struct NestedSteps {
+    static __device__ __forceinline__ void run(F2 &c, const F2 &nP, const F2 &nR, unsigned mask) {
+        const F2 G = fma2(fma2(c, c, nP), c, nR);
+        constexpr unsigned step = (unsigned)(127 - (K + 2)) << 23;              // bits of 2^-(K+2)
+        c = add2(c, F2{signed_step<step>(G.x, mask), signed_step<step>(G.y, mask)});
+        NestedSteps<K + 1, N>::run(c, nP, nR, mask);
+    }
+};
+template <int N>
+struct NestedSteps<N, N> {
+    static __device__ __forceinline__ void run(F2 &, const F2 &, const F2 &, unsigned) {}
+};
+
 template <>
 struct PairSolver<NESTED> {
     static __device__ __forceinline__ F2 reduced_offset(const PairIn &in) {
@@ -294,7 +340,7 @@ struct PairSolver<NESTED> {
         const F2 Wn2 = mul2(W, n2);                                             // x / 3
         const F2 s1 = mul2(n1, n1);
         const F2 t1 = fma2(s1, -1.0f / 3.0f, Wn2);                              // (x - n1^2) / 3
-        const F2 d2 = fma2(n1, 0.5f, sqrt2(max2(fma2(s1, -1.0f / 12.0f, Wn2), 0.0f)));
+        const F2 d2 = fma2(n1, 0.5f, sqrt2(fma2(s1, -1.0f / 12.0f, Wn2)));
         const F2 d1 = ex2_2(fma2(lg2_2(mul2(Wn2, n1)), 1.0f / 3.0f, f2(0.528320834f)));
         F2 d = sel2(lt2(t1, f2(0.0f)), d1, d2);
         const F2 q = mul2(n1, n2);
@@ -305,17 +351,16 @@ struct PairSolver<NESTED> {
         const F2 zero = f2(0.0f);
         const F2 np = sel2(c4, mul2(fma2(q, 4.0f, mul2(ee, -1.0f)), -0.75f), mul2(q, -6.0f));   // -p
         const F2 nr = mul2(q, sel2(c4, mul2(sub2(n3, W), -1.5f), mul2(z, -3.0f)));              // -r
-        F2 lo = sel2(c4, sub2(n3, in.hS), mul2(n1, -1.0f));
+        const F2 lo = sel2(c4, sub2(n3, in.hS), mul2(n1, -1.0f));
         const F2 hi = sel2(c4, zero, min2(e, zero));
-        F2 w = sub2(hi, lo);
-#pragma unroll
-        for (int i = 0; i < 20; ++i) {
-            w = mul2(w, 0.5f);
-            const F2 mid = add2(lo, w);
-            const F2 F = fma2(fma2(mid, mid, np), mid, nr);
-            lo = sel2(gt2(F, zero), mid, lo);
-        }
-        const F2 d34 = max2(add2(sel2(c4, in.hS, n12), fma2(w, 0.5f, lo)), n2);  // floor; drops NaN
+        const F2 w = sub2(hi, lo);
+        const F2 iw = rcp2(w);
+        const F2 iw2 = mul2(iw, iw);
+        const F2 nP = mul2(np, iw2);                                            // -p / w^2
+        const F2 nR = mul2(mul2(nr, iw), iw2);                                  // -r / w^3
+        F2 c = fma2(lo, iw, f2(0.5f));
+        NestedSteps<0, 20>::run(c, nP, nR, kSignMask);
+        const F2 d34 = max2(fma2(c, w, sel2(c4, in.hS, n12)), n2);              // floor; drops NaN
         d = sel2(gt2(t1, mul2(n2, sub2(n2, n1))), d34, d);
         return sel2(le2(n12, W), mul2(add2(W, n12), 0.5f), d);                  // (5)
     }
