@@ -13,24 +13,44 @@ method.  All eight method variants and plic_volume (row a7) are timed the same w
 same run (W warm-up + K timed launches each, CUDA events on the launching stream) and listed
 under "methods"; the headline `value` is the fastest variant that the parity tests hold to
 the 2e-5 bound -- all of them are, see tests/test_parity_gpu.py -- named in config.method.
+`value` is taken in the sustained regime (300 ms of load before the first timed region; on this
+pool a software power cap then holds the SM clocks at 1.5-1.85 GHz); "burst" repeats the headline
+variant after 0.5 s of idle, at full clocks -- the regime MEASURED_PEAKS.json's copy bandwidth
+was taken in.
 
-Multi-GPU (torchrun, one rank per GPU): the path has no exchange step, so rank r solves its
-own 2^26 cells [r 2^26, (r+1) 2^26) of the same seeded stream, no data-path collective;
-`value` = all ranks' cells / max-over-ranks time ("scaling": "weak").
+Per method: `hbm_frac` against the measured copy bandwidth and `hbm_frac_nominal`
+against 8 TB/s; `issue_frac` = warp-instructions per cell (ncu's executed count, from the committed
+table profiles/instruction_counts.txt) x cells/s / (SMs x 4 schedulers x the SM clock sampled in
+that method's timed window); `bound` names the larger of the two fractions.  "stream_ceiling" is the
+same 4-read/1-write stream with no arithmetic (plic_solve with the blank method, d0 = V0 - 1/2);
+"pipe_rates" are the instruction rates of the FMA, SFU and ALU pipes measured in this run
+(plic_pipe_probe), from which the "alu" peak of the compute-bound legs is derived.
 
-"paper_benchmark" is the paper's own benchmark shape (sect. 2.6, Table 3) through
-plic_roundtrip_error: 2^k normals x L = 256 volumes in series per thread, blank run (eq. 33)
-subtracted, ps per PLIC evaluation and E_avg (eq. 32) per method -- compute bound, for
-comparison with the paper's Titan Xp column (context, not the target).
+Other configs of BASELINE.json, each timed like the headline (none is part of `value`):
+"divergence" = configs[2], 2^26 case-stratified cells labelled by the ORACLE (oracle.stratified:
+rejection sampling on the oracle's classifier, V0 by the oracle's forward map), interleaved
+(case = i mod 5: every warp holds all five cases) vs five contiguous blocks, all 8 variants;
+"config4" = configs[3], 2^28 cells, half the normals snapped to an axis or face diagonal,
+V0 ~ Beta(1/2,1/2) (gen.snapped_beta), all 8 variants; "curvature" = plic_curvature on configs[4]
+(256^3 lattice, sphere R = 60), rotating over three copies of the lattice so that no call finds its
+input in L2, with the curvature oracle beside it.  "paper_benchmark" is the paper's own benchmark
+shape (sect. 2.6, Table 3) through plic_roundtrip_error: 2^k normals x L = 256 volumes in series per
+thread, blank run (eq. 33) subtracted, ps per PLIC evaluation and E_avg (eq. 32) per method --
+compute bound, for comparison with the paper's Titan Xp column (context, not the target).
+"storage" lists the fp16-storage and fp64 variants of the solve.
 
-`value` is taken in the sustained regime (300 ms of load before the first timed region; on this pool
-a software power cap then holds the SM clocks at 1.5-1.85 GHz); "burst" repeats the headline variant
-after 0.5 s of idle, at full clocks -- the regime MEASURED_PEAKS.json's copy bandwidth was taken in.
+"e2e" is the same metric through plic_solve_host with pinned HOST buffers (H2D and D2H copies
+inside the timed region), next to the PCIe link's nominal and measured rates.  "cpu_baseline" /
+"cpu_baseline_1core" time the fp64 oracle on all host threads / one thread.
 
-Further objects on the same line (each timed like the headline, none part of `value`):
-"methods" also lists the plane-sphere maps of sect. 3 (8 B per cell); "divergence" times every
-variant on 20 %-per-case cells, interleaved vs contiguous (the purpose of configs[2]); "curvature"
-times plic_curvature on configs[4] (256^3 lattice, sphere R = 60) with the curvature oracle beside it.
+Multi-GPU: the path has no exchange step, so rank r solves its own 2^26 cells
+[r 2^26, (r+1) 2^26) of the same seeded stream, no data-path collective; `value` = all ranks'
+cells / max-over-ranks time ("scaling": "weak").  Under torchrun the ranks come from the
+environment; a plain `python bench.py --gpus N` (N > 1) re-launches itself under
+torch.distributed.run with N ranks on 127.0.0.1.
+
+The last key, "summary", repeats the per-variant results in compact form (drivers that keep only
+the tail of the line still see them).
 
 --impl reference times the fp64 CPU oracle (oracle/), as it stands, on the host cores.
 """
@@ -185,31 +205,35 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------
 # the oracle leg (cpu_baseline and --impl reference)
 # ------------------------------------------------------------------------------------------
-def oracle_rate(arrays, n_cells: int):
+def oracle_rate(arrays, n_cells: int, threads: int = 0):
     """Times oracle.solve on the first n_cells of the workload; returns (cells/s, seconds)."""
     import oracle
     sub = [a[:n_cells] for a in arrays]
     t0 = time.perf_counter()
-    oracle.solve(*sub)
+    oracle.solve(*sub, threads=threads)
     dt = time.perf_counter() - t0
     return n_cells / dt, dt
 
 
-def cpu_baseline(arrays, budget_s: float = 12.0):
-    """The oracle as it stands on all host threads, for about budget_s seconds: a prefix of the
-    workload sized from a calibration pass, repeated when the whole workload takes less."""
+def cpu_baseline(arrays, budget_s: float = 12.0, threads: int = 0):
+    """The oracle as it stands on all host threads (threads=0) or on `threads` of them, for about
+    budget_s seconds: a prefix of the workload sized from a calibration pass, repeated when the
+    whole workload takes less."""
     import oracle
+    all_threads = oracle.max_threads()       # before any call that lowers the OpenMP thread count
     N = arrays[0].shape[0]
-    cal = min(N, 1 << 20)
-    rate, _ = oracle_rate(arrays, cal)                       # calibration (also warms the .so)
+    cal = min(N, 1 << (20 if threads == 0 else 16))
+    rate, _ = oracle_rate(arrays, cal, threads)              # calibration (also warms the .so)
     n = int(min(N, max(cal, rate * budget_s)))
     passes, cells, secs = 0, 0, 0.0
     while passes == 0 or (secs < 0.8 * budget_s and passes < 64):
-        _, dt = oracle_rate(arrays, n)
+        _, dt = oracle_rate(arrays, n, threads)
         passes, cells, secs = passes + 1, cells + n, secs + dt
-    return {"value": cells / secs / 1e9, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
-            "sample": "first %d cells of the workload x %d passes (%.1f s of fp64 bisection, all host "
-                      "threads)" % (n, passes, secs)}
+    cores = all_threads if threads == 0 else threads
+    oracle.solve(arrays[0][:1], arrays[1][:1], arrays[2][:1], arrays[3][:1], threads=all_threads)   # restore
+    return {"value": cells / secs / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "first %d cells of the workload x %d passes (%.1f s of fp64 bisection, %s)" % (
+                n, passes, secs, "all host threads" if threads == 0 else "%d thread(s)" % threads)}
 
 
 def run_reference(args):
@@ -252,6 +276,9 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------
+NOMINAL_HBM_GBS = 8000.0                 # "the nominal 8 TB/s"
+
+
 def measured_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -262,18 +289,38 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md, MEASURED_PEAKS.json absent)"
 
 
-def ncu_traffic(kernel_name: str):
-    """dram bytes per launch of `kernel_name` from the committed ncu summary, or None."""
-    p = os.path.join(ROOT, "profiles", "dram_traffic.txt")
+def profile_table(name):
+    """Rows of a committed profiles/*.txt table: {first column: [other columns]}; '#' lines are
+    comments, a '#@ key value' line is metadata returned under '@key'."""
+    rows = {}
     try:
-        with open(p) as f:
+        with open(os.path.join(ROOT, "profiles", name)) as f:
             for line in f:
                 parts = line.split()
-                if len(parts) >= 2 and parts[0] == kernel_name:
-                    return float(parts[1])
+                if not parts:
+                    continue
+                if parts[0] == "#@" and len(parts) >= 3:
+                    rows["@" + parts[1]] = parts[2:]
+                elif not parts[0].startswith("#"):
+                    rows[parts[0]] = parts[1:]
     except Exception:
         pass
-    return None
+    return rows
+
+
+def ncu_traffic(kernel_name, cells):
+    """(dram bytes per launch, provenance) of `kernel_name` from the committed ncu capture -- only
+    when that capture was taken on the same number of cells, else (None, why)."""
+    t = profile_table("dram_traffic.txt")
+    row = t.get(kernel_name)
+    cap_cells = int(t.get("@cells", ["0"])[0])
+    src = "profiles/dram_traffic.txt (ncu --set full, commit %s, %d cells per launch)" % (
+        t.get("@commit", ["?"])[0], cap_cells)
+    if row is None:
+        return None, "no ncu capture of this kernel in profiles/dram_traffic.txt"
+    if cap_cells != cells:
+        return None, "ncu capture is for %d cells per launch, this run uses %d" % (cap_cells, cells)
+    return float(row[0]), src
 
 
 def time_launches(fn, steps, warmup, stream):
@@ -299,6 +346,48 @@ def time_launches(fn, steps, warmup, stream):
     return e0.elapsed_time(e1), (w0, w1)
 
 
+def pcie_link(sampler):
+    """Nominal PCIe rate of the GPU's link from NVML (GB/s per direction), or None."""
+    try:
+        nv, h = sampler.nv, sampler.h
+        gen_, width = nv.nvmlDeviceGetCurrPcieLinkGeneration(h), nv.nvmlDeviceGetCurrPcieLinkWidth(h)
+        per_lane = {1: 0.25, 2: 0.5, 3: 0.985, 4: 1.969, 5: 3.938, 6: 7.563}.get(int(gen_))
+        return {"gen": int(gen_), "width": int(width), "nominal_gbs_per_direction": per_lane * width if per_lane else None}
+    except Exception:
+        return None
+
+
+VARIANTS = [(m, f) for f in (True, False) for m in ("analytic", "sz", "newton", "nested")]
+
+
+def time_variants(plic, arrays, out, steps, warmup, stream, world, sampler, sms, counts, peak):
+    """Times the eight plic_solve variants on `arrays`; one dict per variant with both HBM fractions,
+    the issue fraction at the clock sampled in its own window, and the binding roofline."""
+    N = arrays[0].numel()
+    res = {}
+    for m, f in VARIANTS:
+        name = plic.plic_method_name(plic.method_id(m, f))
+        c0 = plic.plic_launch_count()
+        ms, win = time_launches(lambda: plic.plic_solve(*arrays, out=out, method=m, fast=f), steps, warmup, stream)
+        launches = (plic.plic_launch_count() - c0) - warmup
+        ms = max_over_ranks(ms) / steps
+        clk = sampler.summary([win])
+        gbs = BYTES_PER_CELL * N / (ms * 1e-3) / 1e9
+        e = {"value": N * world / (ms * 1e-3) / 1e9, "ms_per_step": ms, "launches": launches,
+             "bytes_per_cell": BYTES_PER_CELL, "hbm_gbs_per_gpu": gbs, "hbm_frac": gbs / peak,
+             "hbm_frac_nominal": gbs / NOMINAL_HBM_GBS, "sm_mhz": clk.get("sm_mhz")}
+        e["roofline_frac"] = e["hbm_frac"]
+        row = counts.get(name)
+        if row is not None and clk.get("sm_mhz"):
+            wipc = float(row[0])
+            e["warp_inst_per_cell"] = wipc
+            e["lanes_per_inst"] = float(row[1])
+            e["issue_frac"] = wipc * N / (ms * 1e-3) / (sms * 4 * clk["sm_mhz"] * 1e6)
+            e["bound"] = "issue" if e["issue_frac"] > e["hbm_frac"] else "hbm"
+        res[name] = e
+    return res
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -316,62 +405,114 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     import paper_2006_12838_b200 as plic           # raises if libplic.so cannot be built/loaded
 
+    sms = torch.cuda.get_device_properties(local).multi_processor_count
     N = 1 << args.log2n
     lo, hi = rank_cells(N, rank)
     host = gen.random_sphere(N, SEED, start=lo)                       # fp32 V0, nx, ny, nz
     dV, dx, dy, dz = [torch.from_numpy(a).cuda() for a in host]
     out = torch.empty_like(dV)
     stream = torch.cuda.current_stream()
+    peak, peak_src = measured_peak()
+    counts = profile_table("instruction_counts.txt")
 
-    variants = [(m, f) for f in (True, False) for m in ("analytic", "sz", "newton", "nested")]
-    solve_names_all = [m + ("-fast" if f else "") for m, f in variants]
-    sampler = ClockSampler(local)
+    sampler = ClockSampler(local, period_s=0.002)
     sampler.start()
 
-    # bring the clocks up before any timing (not counted as warm-up steps)
+    # bring the clocks into the sustained regime before any timing (not counted as warm-up steps)
     t_end = time.perf_counter() + args.prewarm_ms / 1e3
     while time.perf_counter() < t_end:
         for _ in range(20):
             plic.plic_solve(dV, dx, dy, dz, out=out, method="analytic", fast=True)
         torch.cuda.synchronize()
 
-    methods = {}
-    windows = {}
     launches_before = plic.plic_launch_count()
-    for m, f in variants:
-        name = plic.plic_method_name(plic.method_id(m, f))
-        c0 = plic.plic_launch_count()
-        ms, win = time_launches(lambda: plic.plic_solve(dV, dx, dy, dz, out=out, method=m, fast=f),
-                                args.steps, args.warmup, stream)
-        timed_launches = (plic.plic_launch_count() - c0) - args.warmup
-        ms = max_over_ranks(ms)
-        grid, block, cpt = plic.plic_launch_config(m, N, f)
-        gcs = N * world * args.steps / (ms * 1e-3) / 1e9
-        methods[name] = {"value": gcs, "ms_per_step": ms / args.steps, "launches": timed_launches,
-                         "hbm_gbs_per_gpu": BYTES_PER_CELL * N * args.steps / (ms * 1e-3) / 1e9,
-                         "grid": grid, "block": block}
-        windows[name] = win
+    windows = {}
+    methods = time_variants(plic, (dV, dx, dy, dz), out, args.steps, args.warmup, stream, world, sampler, sms,
+                            counts, peak)
+
+    def timed_map(name, fn, bytes_per_cell):
+        ms, win = time_launches(fn, args.steps, args.warmup, stream)
+        ms = max_over_ranks(ms) / args.steps
+        gbs = bytes_per_cell * N / (ms * 1e-3) / 1e9
+        clk = sampler.summary([win])
+        e = {"value": N * world / (ms * 1e-3) / 1e9, "ms_per_step": ms, "launches": args.steps,
+             "bytes_per_cell": bytes_per_cell, "hbm_gbs_per_gpu": gbs, "hbm_frac": gbs / peak,
+             "hbm_frac_nominal": gbs / NOMINAL_HBM_GBS, "roofline_frac": gbs / peak, "sm_mhz": clk.get("sm_mhz")}
+        row = counts.get(name)
+        if row is not None and clk.get("sm_mhz"):
+            e["warp_inst_per_cell"] = float(row[0])
+            e["issue_frac"] = float(row[0]) * N / (ms * 1e-3) / (sms * 4 * clk["sm_mhz"] * 1e6)
+            e["bound"] = "issue" if e["issue_frac"] > e["hbm_frac"] else "hbm"
+        return e
+
+    # the 4-read / 1-write stream with no arithmetic, in the same sustained regime
+    stream_ceiling = timed_map("blank", lambda: plic.plic_solve(dV, dx, dy, dz, out=out, method="blank"), BYTES_PER_CELL)
+    stream_ceiling["what"] = ("plic_solve with PLIC_METHOD_BLANK (d0 = V0 - 1/2): the same four input streams, "
+                              "body kernel and launch geometry as the HBM-bound solvers, no arithmetic")
     vol = torch.empty_like(dV)
-    ms, win = time_launches(lambda: plic.plic_volume(out, dx, dy, dz, out=vol),
-                            args.steps, args.warmup, stream)
-    ms = max_over_ranks(ms)
-    methods["plic_volume"] = {"value": N * world * args.steps / (ms * 1e-3) / 1e9,
-                              "ms_per_step": ms / args.steps, "launches": args.steps,
-                              "hbm_gbs_per_gpu": BYTES_PER_CELL * N * args.steps / (ms * 1e-3) / 1e9}
-    windows["plic_volume"] = win
+    methods["plic_volume"] = timed_map("plic_volume", lambda: plic.plic_volume(out, dx, dy, dz, out=vol), BYTES_PER_CELL)
     # plane-sphere maps of sect. 3: one array in, one out (8 B per cell)
-    sphere_names = []
     for name, fn in (("sphere_solve-fast", lambda: plic.plic_sphere_solve(dV, out=out, fast=True)),
                      ("sphere_solve", lambda: plic.plic_sphere_solve(dV, out=out, fast=False)),
                      ("sphere_volume", lambda: plic.plic_sphere_volume(out, out=vol))):
-        ms, win = time_launches(fn, args.steps, args.warmup, stream)
-        ms = max_over_ranks(ms)
-        methods[name] = {"value": N * world * args.steps / (ms * 1e-3) / 1e9,
-                         "ms_per_step": ms / args.steps, "launches": args.steps, "bytes_per_cell": 8,
-                         "hbm_gbs_per_gpu": 8 * N * args.steps / (ms * 1e-3) / 1e9}
-        windows[name] = win
-        sphere_names.append(name)
+        methods[name] = timed_map(name, fn, 8)
+
+    # ---- fp16-storage and fp64 variants of the solve ----------------------------
+    storage = None
+    if hasattr(plic, "plic_solve_h") and not args.no_storage:
+        storage = {}
+        hV, hx, hy, hz = [t.half() for t in (dV, dx, dy, dz)]
+        hout = torch.empty_like(hV)
+        for m in ("analytic", "sz", "newton", "nested"):
+            storage["%s-fast/f16" % m] = timed_map(
+                "%s-fast/f16" % m, lambda: plic.plic_solve_h(hV, hx, hy, hz, out=hout, method=m), 10)
+        storage["analytic-fast/f16in-f32out"] = timed_map(
+            "analytic-fast/f16in-f32out", lambda: plic.plic_solve_h(hV, hx, hy, hz, out=out, method="analytic"), 12)
+        del hV, hx, hy, hz, hout
+        fV, fx, fy, fz = [t.double() for t in (dV, dx, dy, dz)]
+        fout = torch.empty_like(fV)
+        for m in ("analytic", "sz"):
+            storage["%s/f64" % m] = timed_map("%s/f64" % m, lambda: plic.plic_solve_f64(fV, fx, fy, fz, out=fout, method=m), 40)
+        del fV, fx, fy, fz, fout
     total_launches = plic.plic_launch_count() - launches_before
+
+    solve_names = [plic.plic_method_name(plic.method_id(m, f)) for m, f in VARIANTS]
+    head = args.method if args.method != "auto" else max(solve_names, key=lambda k: methods[k]["value"])
+    H = methods[head]
+    hm, hf = (head[:-5], True) if head.endswith("-fast") else (head, False)
+    # the headline once more for its clock window (the per-method windows are not kept)
+    _, head_win = time_launches(lambda: plic.plic_solve(dV, dx, dy, dz, out=out, method=hm, fast=hf),
+                                args.steps, args.warmup, stream)
+    windows[head] = head_win
+
+    # ---- instruction rates of the pipes, measured here ("confirm with an FFMA-only and a
+    # MUFU-only microbenchmark"): warp-instructions per sub-partition per clock at the sampled clock
+    pipe_rates = None
+    if not args.no_probes:
+        sink = torch.zeros(256, device="cuda")
+        pipe_rates = {"unit": "warp-instructions per SM sub-partition per clock", "sms": sms, "probes": {}}
+        torch.cuda.synchronize()
+        time.sleep(0.3)                                  # the probes run at whatever clock they draw themselves
+        for name in plic.PROBES:
+            def probe(trips):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                w0 = time.perf_counter()
+                e0.record(stream)
+                n_inst = plic.plic_pipe_probe(name, trips, sink)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                return n_inst, e0.elapsed_time(e1) * 1e-3, (w0, time.perf_counter())
+            probe(200)
+            _, cal, _ = probe(400)                       # size the timed launch to ~30 ms: >= 10 clock samples
+            n_inst, sec, win = probe(max(400, int(400 * 0.030 / max(cal, 1e-6))))
+            ins = [s_[1] for s_ in sampler.samples if win[0] + 0.004 <= s_[0] <= win[1]]
+            mhz = sorted(ins)[len(ins) // 2] if ins else (sampler.sm_max or 1965)
+            pipe_rates["probes"][name] = {"t_inst_per_s": n_inst / sec / 1e12, "sm_mhz": mhz, "ms": sec * 1e3,
+                                          "per_smsp_clk": n_inst / sec / (sms * 4 * mhz * 1e6)}
+        pipe_rates["reading"] = ("scalar FFMA/FADD/FMUL issue at ~1 per clock, packed fp32x2 and every ALU-pipe "
+                                 "instruction (min/max, compare, select, logic) at 1 per 2 clocks, MUFU at 1 per 8; "
+                                 "nested_step* = one halving of nested-fast for a pair of cells in three encodings")
+        del sink
 
     # ---- the paper's own benchmark shape (sect. 2.6, Table 3): compute bound, blank run subtracted
     paper = None
@@ -382,11 +523,12 @@ def run_ours(args):
         paper = {"normals": PN, "L": PL, "unit": "ps per PLIC evaluation, blank run (eq. 33) subtracted",
                  "paper_titan_xp_ps": {"sz": 12.8, "kawano": 16.0, "analytic": 19.0, "newton": 19.2, "nested": 106.4},
                  "methods": {}}
-        pnames = ["blank"] + solve_names_all + ["kawano"]
+        pnames = ["blank"] + solve_names + ["kawano"]
         raw = {}
+        pwin = {}
         for name in pnames:
-            ms, _ = time_launches(lambda: plic.plic_roundtrip_error(*pn, PL, out=pE, method=name),
-                                  3, 3, stream)
+            ms, pwin[name] = time_launches(lambda: plic.plic_roundtrip_error(*pn, PL, out=pE, method=name),
+                                           3, 3, stream)
             raw[name] = (max_over_ranks(ms) / 3, float(pE.double().mean()))
         for name in pnames:
             ms, eavg = raw[name]
@@ -394,119 +536,142 @@ def run_ours(args):
             paper["methods"][name] = {"ms": ms, "ps_per_eval": (ms - raw["blank"][0]) * 1e9 / (PN * PL),
                                       "ps_per_eval_incl_blank": ms * 1e9 / (PN * PL),
                                       "E_avg": None if nan else eavg, "E_avg_is_nan": nan}
-        # issue roofline of the compute-bound loop: thread-instructions per (solve + forward map)
-        # evaluation from the committed ncu capture (profiles/r01_ncu_summary.md, 2c) x evaluations/s,
-        # against 148 SMs x 4 schedulers x 32 lanes x the max SM clock
-        ipe = 78.0
-        sm_max = (sampler.sm_max or 1965) * 1e6
-        peak_tis = 148 * 4 * 32 * sm_max / 1e12
-        ach = ipe * PN * PL / (raw["analytic-fast"][0] * 1e-3) / 1e12
-        paper["roofline"] = {"bound": "alu", "kernel": "roundtrip_kernel<analytic, fast>", "achieved": ach,
-                             "peak": peak_tis, "unit": "T thread-instructions/s", "frac": ach / peak_tis,
-                             "thread_instructions_per_evaluation": ipe,
-                             "peak_source": "148 SMs x 4 x 32 lanes x max SM clock (issue port; DESIGN.md 6)"}
+        # issue roofline of the compute-bound loop: warp-instructions per (solve + forward map) evaluation
+        # from the committed ncu capture x evaluations/s, against SMs x 4 x the clock sampled in the window
+        row = counts.get("roundtrip:analytic-fast")
+        mhz = sampler.summary([pwin["analytic-fast"]]).get("sm_mhz") or sampler.sm_max or 1965
+        if row is not None:
+            wipe = float(row[0])
+            peak_wis = sms * 4 * mhz * 1e6 / 1e12
+            ach = wipe * PN * PL / (raw["analytic-fast"][0] * 1e-3) / 1e12
+            paper["roofline"] = {"bound": "alu", "kernel": "roundtrip_kernel<analytic, fast>", "achieved": ach,
+                                 "peak": peak_wis, "unit": "T warp-instructions/s", "frac": ach / peak_wis,
+                                 "warp_instructions_per_evaluation": wipe, "sm_mhz": mhz,
+                                 "counts_source": "profiles/instruction_counts.txt (ncu smsp__inst_executed.sum, commit %s)"
+                                                  % counts.get("@commit", ["?"])[0],
+                                 "peak_source": "%d SMs x 4 schedulers x 1 warp-instruction per clock at the sampled SM "
+                                                "clock; the scalar-FFMA probe of this run reaches %.2f of it, packed and "
+                                                "ALU-pipe instructions half of it (pipe_rates)" % (
+                                                    sms, pipe_rates["probes"]["ffma"]["per_smsp_clk"] if pipe_rates else float("nan"))}
         del pn, pE
 
-    solve_names = [plic.plic_method_name(plic.method_id(m, f)) for m, f in variants]
-    head = args.method if args.method != "auto" else max(solve_names, key=lambda k: methods[k]["value"])
-    H = methods[head]
-    peak, peak_src = measured_peak()
     for k, v in methods.items():
-        v["roofline_frac"] = v["hbm_gbs_per_gpu"] / peak
+        v.setdefault("roofline_frac", v["hbm_frac"])
 
-    # ---- divergence cost (the purpose of configs[2]): the same cells, 20 % per intersection case,
-    # once interleaved (case = i mod 5: every warp holds all five cases) and once in five contiguous
-    # blocks (every warp holds one case).  The case label is read off the solved offset.
+    # ---- divergence cost = BASELINE.json configs[2]: 2^26 case-stratified cells labelled by the oracle
+    # (rejection sampling on the oracle's classifier, V0 by the oracle's forward map), once interleaved
+    # (case = i mod 5: every warp holds all five cases) and once in five contiguous blocks
     diverg = None
-    if not args.no_divergence and N >= (1 << 24):
-        per = min(1 << 22, N // 32)
-        d0 = plic.plic_solve(dV, dx, dy, dz, method="analytic", fast=False)
-        srt, _ = torch.sort(torch.stack([dx.abs(), dy.abs(), dz.abs()]), dim=0)
-        n1, n2, n3 = srt[0], srt[1], srt[2]
-        dd = 0.5 * (n1 + n2 + n3) - d0.abs()
-        case = torch.where(dd >= n1 + n2, 5, torch.where(dd < n1, 1, torch.where(dd <= n2, 2,
-                           torch.where(dd <= n3, 3, 4))))
-        del srt, n1, n2, n3, dd, d0
-        picks = [torch.nonzero(case == c).flatten()[:per] for c in (1, 2, 3, 4, 5)]
-        del case
-        if all(p.numel() == per for p in picks):
-            contiguous = torch.cat(picks)
-            interleaved = torch.stack(picks, dim=1).flatten()
-            diverg = {"cells": 5 * per, "layout": "20 % per case; interleaved (i mod 5) vs five contiguous blocks",
-                      "source": "the first %d cells of each case among the workload's cells" % per,
-                      "l2": "%.0f MB touched per launch vs 126 MB of L2" % (20 * 5 * per / 1e6), "methods": {}}
-            sets = {}
-            for lay, idx in (("interleaved", interleaved), ("contiguous", contiguous)):
-                sets[lay] = [t[idx].contiguous() for t in (dV, dx, dy, dz)]
-            o5 = torch.empty(5 * per, device="cuda")
-            for m, f in variants:
-                name = plic.plic_method_name(plic.method_id(m, f))
-                r = {}
-                for lay in ("interleaved", "contiguous"):
-                    a = sets[lay]
-                    ms, _ = time_launches(lambda: plic.plic_solve(*a, out=o5, method=m, fast=f),
-                                          args.steps, args.warmup, stream)
-                    r[lay + "_ms"] = max_over_ranks(ms) / args.steps
-                r["interleaved_over_contiguous"] = r["interleaved_ms"] / r["contiguous_ms"]
-                diverg["methods"][name] = r
-            del sets, o5, contiguous, interleaved
-        del picks
+    if not args.no_divergence and args.log2n >= 20:
+        from oracle.stratified import stratified, SEED as STRAT_SEED
+        t0 = time.perf_counter()
+        # torchrun sets OMP_NUM_THREADS=1 per rank: give the generator this rank's share of the cores
+        sV, sx, sy, sz, kase = stratified(N, STRAT_SEED, start=lo, threads=max(1, (os.cpu_count() or 1) // world))
+        gen_s = time.perf_counter() - t0
+        order = np.concatenate([np.arange((k - lo) % 5, N, 5) for k in range(5)])
+        diverg = {"workload": "configs[2]: N=2^%d case-stratified, seed 2, 20 %% per intersection case; labels and V0 "
+                              "from the oracle (oracle/stratified.c)" % args.log2n,
+                  "cells": N, "case_counts": np.bincount(kase, minlength=6)[1:].tolist(),
+                  "layouts": "interleaved (case = i mod 5 + 1) vs five case-contiguous blocks of the same cells",
+                  "generator_s": gen_s, "methods": {}}
+        r = {}
+        for lay in ("interleaved", "contiguous"):
+            a = [torch.from_numpy(t if lay == "interleaved" else t[order]).cuda() for t in (sV, sx, sy, sz)]
+            r[lay] = time_variants(plic, a, out, args.steps, args.warmup, stream, world, sampler, sms, counts, peak)
+            del a
+        for name in solve_names:
+            i_, c_ = r["interleaved"][name], r["contiguous"][name]
+            diverg["methods"][name] = {"interleaved_ms": i_["ms_per_step"], "contiguous_ms": c_["ms_per_step"],
+                                       "interleaved_over_contiguous": i_["ms_per_step"] / c_["ms_per_step"],
+                                       "interleaved_hbm_frac": i_["hbm_frac"], "contiguous_hbm_frac": c_["hbm_frac"]}
+        del sV, sx, sy, sz, kase, order, r
+
+    # ---- BASELINE.json configs[3]: 2^28 cells, snapped normals, V0 ~ Beta(1/2, 1/2); the large-batch regime
+    config4 = None
+    if not args.no_config4:
+        N4 = 1 << args.config4_log2n
+        t0 = time.perf_counter()
+        h4 = gen.snapped_beta(N4, 3, start=rank * N4)
+        gen_s = time.perf_counter() - t0
+        a4 = [torch.from_numpy(t).cuda() for t in h4]
+        del h4
+        o4 = torch.empty_like(a4[0])
+        r4 = time_variants(plic, a4, o4, args.steps, args.warmup, stream, world, sampler, sms, counts, peak)
+        config4 = {"workload": "configs[3]: N=2^%d cells (%.1f GB in, %.1f GB out), seed 3, half the normals snapped to an "
+                               "axis or a face diagonal, V0 ~ Beta(1/2,1/2)" % (args.config4_log2n, 16 * N4 / 1e9, 4 * N4 / 1e9),
+                   "cells": N4, "generator_s": gen_s, "methods": r4}
+        del a4, o4
 
     # ---- curvature on configs[4]: 256^3 lattice, sphere R = 60 (sect. 4; two launches per call) ----
     curv = None
     if not args.no_curvature:
         R5 = 60.0
-        phi5 = torch.from_numpy(gen.sphere_fill_lattice(256, R5, (128.3, 127.7, 128.1), 8)).cuda()
-        kap5 = torch.empty_like(phi5)
-        work5 = torch.empty(1 + phi5.numel(), dtype=torch.int32, device="cuda")
+        host_phi = gen.sphere_fill_lattice(256, R5, (128.3, 127.7, 128.1), 8)
+        # three copies of the lattice, used in turn: 3 x (67 MB read + 67 MB written) > 126 MB of L2,
+        # so no call finds its input in cache
+        phis = [torch.from_numpy(host_phi).cuda() for _ in range(3)]
+        kaps = [torch.empty_like(p_) for p_ in phis]
+        work5 = torch.empty(1 + phis[0].numel(), dtype=torch.int32, device="cuda")
+        turn = [0]
+
+        def curv_call():
+            j = turn[0] % 3
+            turn[0] += 1
+            plic.plic_curvature(phis[j], out=kaps[j], work=work5)
         c0 = plic.plic_launch_count()
-        ms, _ = time_launches(lambda: plic.plic_curvature(phi5, out=kap5, work=work5), args.steps,
-                              args.warmup, stream)
+        ms, _ = time_launches(curv_call, args.steps, args.warmup, stream)
         per_call = (plic.plic_launch_count() - c0) / (args.steps + args.warmup)
         ms = max_over_ranks(ms) / args.steps
         n_if = int(work5[0].item())
+        kap5 = kaps[0]
         kk = -kap5[kap5 != 0].double() * R5
+        ncell = phis[0].numel()
         curv = {"workload": "configs[4]: 256^3 lattice, sphere R=60 at (128.3,127.7,128.1), phi = fraction "
-                            "of 8^3 sub-cell points inside", "ms_per_call": ms, "launches_per_call": per_call,
-                "lattice_gcells_per_s": phi5.numel() / (ms * 1e-3) / 1e9, "interface_points": n_if,
+                            "of 8^3 sub-cell points inside; three lattice copies used in turn (L2-cold input)",
+                "ms_per_call": ms, "launches_per_call": per_call,
+                "lattice_gcells_per_s": ncell / (ms * 1e-3) / 1e9, "interface_points": n_if,
                 "interface_mpoints_per_s": n_if / (ms * 1e-3) / 1e6,
-                "hbm_gbs": 8 * phi5.numel() / (ms * 1e-3) / 1e9,
-                "roofline_frac": 8 * phi5.numel() / (ms * 1e-3) / 1e9 / measured_peak()[0],
-                "bytes_per_lattice_cell": 8, "minus_kappa_R_mean": float(kk.mean()),
+                "hbm_gbs": 8 * ncell / (ms * 1e-3) / 1e9,
+                "roofline_frac": 8 * ncell / (ms * 1e-3) / 1e9 / peak,
+                "hbm_frac_nominal": 8 * ncell / (ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+                "bytes_per_lattice_cell": 8, "all_interface_kappa_finite": bool(torch.isfinite(kap5).all()),
+                "minus_kappa_R_mean": float(kk.mean()),
                 "L1_error_eq50": float((kk - 1.0).abs().mean())}
         if not args.no_cpu_baseline and world == 1 and rank == 0:
             # the curvature oracle (numpy fp64 + the bisection oracle) on the same lattice, once
             from oracle import curvature as ocurv
             import oracle as _o
-            host_phi = phi5.cpu().numpy()
             t0 = time.perf_counter()
             ocurv.curvature_lattice(host_phi)
             dt = time.perf_counter() - t0
             curv["cpu_baseline"] = {"value": n_if / dt / 1e6, "unit": "M interface points/s",
                                     "cores": _o.max_threads(), "kind": "oracle",
                                     "sample": "the whole 256^3 lattice once (%.1f s)" % dt}
-        del phi5, kap5, work5
+        del phis, kaps, work5, host_phi
 
-    # ---- the headline variant once more after an idle gap: the clocks recover from the power cap,
-    # which is the regime MEASURED_PEAKS.json's burst figure was taken in (reported beside `value`,
-    # which stays the sustained number)
-    hm0, hf0 = (head[:-5], True) if head.endswith("-fast") else (head, False)
+    # ---- the headline variant and the blank stream once more after an idle gap: the clocks recover from
+    # the power cap, which is the regime MEASURED_PEAKS.json's burst figure was taken in (reported beside
+    # `value`, which stays the sustained number)
     torch.cuda.synchronize()
     time.sleep(0.5)
     bsteps = max(1, min(args.steps, 30))
-    ms, bwin = time_launches(lambda: plic.plic_solve(dV, dx, dy, dz, out=out, method=hm0, fast=hf0),
+    ms, bwin = time_launches(lambda: plic.plic_solve(dV, dx, dy, dz, out=out, method=hm, fast=hf),
                              bsteps, args.warmup, stream)
     ms = max_over_ranks(ms) / bsteps
     burst = {"method": head, "steps": bsteps, "ms_per_step": ms, "value": N * world / (ms * 1e-3) / 1e9,
              "unit": UNIT, "hbm_gbs_per_gpu": BYTES_PER_CELL * N / (ms * 1e-3) / 1e9,
              "roofline_frac": BYTES_PER_CELL * N / (ms * 1e-3) / 1e9 / peak,
              "note": "same kernel, timed after 0.5 s of idle (no sustained load before it)"}
+    time.sleep(0.5)
+    ms, _ = time_launches(lambda: plic.plic_solve(dV, dx, dy, dz, out=out, method="blank"), bsteps, args.warmup, stream)
+    burst["stream_ceiling_ms"] = max_over_ranks(ms) / bsteps
+    burst["stream_ceiling_gbs"] = BYTES_PER_CELL * N / (burst["stream_ceiling_ms"] * 1e-3) / 1e9
+    burst["frac_of_stream_ceiling"] = burst["stream_ceiling_ms"] / burst["ms_per_step"]
 
     # ---- end to end through the host-array C ABI: pinned host buffers, copies inside ----------
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     pin = [torch.from_numpy(a).pin_memory() for a in host]
     pout = torch.empty(N, dtype=torch.float32).pin_memory()
-    hm, hf = (head[:-5], True) if head.endswith("-fast") else (head, False)
     for _ in range(2):
         plic.plic_solve_host(*pin, out=pout, method=hm, fast=hf)
     torch.cuda.synchronize()
@@ -521,13 +686,25 @@ def run_ours(args):
     e2e_s = max_over_ranks(t1 - t0)
     plic.plic_solve(dV, dx, dy, dz, out=out, method=hm, fast=hf)
     e2e_same = bool(np.array_equal(pout.numpy(), out.cpu().numpy()))   # host API == device API, bitwise
+    # the link itself: one pinned array up, one down, CUDA events
+    link = pcie_link(sampler) or {}
+    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    e0.record(stream)
+    dV.copy_(pin[0], non_blocking=True)
+    e1.record(stream)
+    pout.copy_(out, non_blocking=True)
+    e2.record(stream)
+    torch.cuda.synchronize()
+    link["measured_h2d_gbs"] = 4 * N / (e0.elapsed_time(e1) * 1e-3) / 1e9
+    link["measured_d2h_gbs"] = 4 * N / (e1.elapsed_time(e2) * 1e-3) / 1e9
     sampler.stop()
     plic.plic_host_release()
 
     clocks = sampler.summary([windows[head]])
     if rank == 0:
-        traffic = ncu_traffic(head)
+        traffic, traffic_src = ncu_traffic(head, N)
         achieved = H["hbm_gbs_per_gpu"]
+        per_step_s = e2e_s / e2e_steps
         line = {
             "metric": METRIC, "value": H["value"], "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": H["ms_per_step"],
@@ -537,34 +714,65 @@ def run_ours(args):
                        "headline_rule": "fastest of the 8 plic_solve variants" if args.method == "auto"
                        else "--method",
                        "l2": "inputs larger than L2 (1.07 GB read + 0.27 GB written per step vs 126 MB)",
-                       "prewarm_ms": args.prewarm_ms, "launch": {"grid": H["grid"], "block": H["block"],
-                                                                 "cells_per_thread": 4}},
+                       "prewarm_ms": args.prewarm_ms, "launch": {"grid": plic.plic_launch_config(hm, N, hf)[0],
+                                                                 "block": 256, "cells_per_thread": 4}},
             "clocks": clocks,
             "gpu_launches": H["launches"],
             "gpu_launches_all_timed_regions": total_launches,
             "e2e": {"value": N * world * e2e_steps / e2e_s / 1e9, "unit": UNIT,
                     "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 4 * N, "steps": e2e_steps,
-                    "launches": e2e_launches, "matches_device_api_bitwise": e2e_same, "api": "plic_solve_host (pinned host arrays, chunked "
-                    "H2D/kernel/D2H pipeline inside libplic)", "timer": "host wall clock around the "
-                    "synchronous calls, device synchronised on both sides"},
+                    "launches": e2e_launches, "matches_device_api_bitwise": e2e_same,
+                    "h2d_gbs": 16 * N / per_step_s / 1e9, "d2h_gbs": 4 * N / per_step_s / 1e9,
+                    "pcie": link,
+                    "bound": "the host link: both directions run concurrently, so the step cannot be shorter than "
+                             "16 B/cell over the H2D rate; frac_of_link = achieved H2D rate / measured pinned H2D rate",
+                    "frac_of_link": (16 * N / per_step_s / 1e9) / link["measured_h2d_gbs"],
+                    "api": "plic_solve_host (pinned host arrays, chunked H2D/kernel/D2H pipeline inside libplic)",
+                    "timer": "host wall clock around the synchronous calls, device synchronised on both sides"},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": traffic, "kernel": head,
+                         "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "kernel": head,
+                         "frac_nominal": achieved / NOMINAL_HBM_GBS, "peak_nominal": NOMINAL_HBM_GBS,
+                         "frac_of_stream_ceiling": stream_ceiling["ms_per_step"] / H["ms_per_step"],
+                         "issue_frac": H.get("issue_frac"),
                          "algorithmic_bytes_per_launch": BYTES_PER_CELL * N, "peak_source": peak_src,
                          "peak_note": "the measured peak is a copy (1 read : 1 write); this stream is 4 reads : "
-                                      "1 write and a blank kernel of the same shape reaches 6.8-7.1 TB/s "
-                                      "(DESIGN.md section 6), so frac can exceed 1"},
+                                      "1 write, whose own ceiling in this run is stream_ceiling (a blank kernel of the "
+                                      "same shape), so frac can exceed 1"},
+            "stream_ceiling": stream_ceiling,
             "methods": methods,
         }
         burst["clocks"] = sampler.summary([bwin])
         line["burst"] = burst
+        if storage is not None:
+            line["storage"] = storage
+        if pipe_rates is not None:
+            line["pipe_rates"] = pipe_rates
         if paper is not None:
             line["paper_benchmark"] = paper
         if curv is not None:
             line["curvature"] = curv
         if diverg is not None:
             line["divergence"] = diverg
+        if config4 is not None:
+            line["config4"] = config4
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(host)
+            line["cpu_baseline_1core"] = cpu_baseline(host, budget_s=4.0, threads=1)
+        # compact repeat of the per-variant results, last on the line
+        r3 = lambda x: None if x is None else round(x, 3)
+        line["summary"] = {
+            "cols": "ms, hbm_frac, issue_frac, bound | config3 interleaved ms, interleaved/contiguous | config4 ms, hbm_frac",
+            "rows": {k: [round(methods[k]["ms_per_step"], 4), r3(methods[k]["hbm_frac"]), r3(methods[k].get("issue_frac")),
+                         methods[k].get("bound"),
+                         None if diverg is None else round(diverg["methods"][k]["interleaved_ms"], 4),
+                         None if diverg is None else r3(diverg["methods"][k]["interleaved_over_contiguous"]),
+                         None if config4 is None else round(config4["methods"][k]["ms_per_step"], 4),
+                         None if config4 is None else r3(config4["methods"][k]["hbm_frac"])] for k in solve_names},
+            "stream_ceiling_ms": round(stream_ceiling["ms_per_step"], 4),
+            "plic_volume_ms": round(methods["plic_volume"]["ms_per_step"], 4),
+            "curvature_ms": None if curv is None else round(curv["ms_per_call"], 4),
+            "storage_ms": None if storage is None else {k: round(v["ms_per_step"], 4) for k, v in storage.items()},
+        }
         print(json.dumps(line), flush=True)
     if world > 1:
         import torch.distributed as dist
@@ -573,7 +781,49 @@ def run_ours(args):
     return 0
 
 
+def run_plumbing_only(args):
+    """The multi-rank plumbing of this file without a GPU (CPU test of `--gpus N`): rendezvous on gloo,
+    each rank generates a slice of its own cell range, the per-rank timings are MAX-reduced, rank 0
+    prints one JSON line.  No PLIC arithmetic is done and no metric is reported."""
+    import numpy as np
+    import torch.distributed as dist
+    import gen
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("gloo")
+    per = 1 << 12
+    lo, hi = rank_cells(per, rank)
+    shard = gen.random_sphere(hi - lo, SEED, start=lo)
+    t = max_over_ranks(1.0 + rank, device="cpu")
+    total = sum_over_ranks(float(hi - lo), device="cpu")
+    check = sum_over_ranks(float(np.sum(shard[0], dtype=np.float64)), device="cpu")
+    if rank == 0:
+        print(json.dumps({"plumbing_only": True, "n_gpus": world, "ranks": world, "cells": int(total),
+                          "max_over_ranks": t, "checksum": check}), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def relaunch_with_ranks(args, argv):
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: start N ranks of this file
+    under torch.distributed.run on 127.0.0.1 and pass its exit code on."""
+    import socket
+    import subprocess
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+    return subprocess.call(cmd)
+
+
 def main(argv=None):
+    argv = sys.argv[1:] if argv is None else list(argv)
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=100)
@@ -585,13 +835,23 @@ def main(argv=None):
     ap.add_argument("--prewarm-ms", type=float, default=300.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-curvature", action="store_true", help="skip the plic_curvature leg")
-    ap.add_argument("--no-divergence", action="store_true", help="skip the case-stratified divergence leg")
+    ap.add_argument("--no-divergence", action="store_true", help="skip the configs[2] (case-stratified) leg")
+    ap.add_argument("--no-config4", action="store_true", help="skip the configs[3] (2^28 snapped/Beta) leg")
+    ap.add_argument("--config4-log2n", type=int, default=28)
+    ap.add_argument("--no-probes", action="store_true", help="skip the instruction-rate probes")
+    ap.add_argument("--no-storage", action="store_true", help="skip the fp16-storage / fp64 variants")
+    ap.add_argument("--plumbing-only", action="store_true",
+                    help="exercise the multi-rank launch and reductions on CPU (gloo); no GPU work, no metric")
     ap.add_argument("--paper-log2n", type=int, default=24,
                     help="normals in the paper-shaped compute-bound leg = 2^k, L = 256 volumes each "
                          "(the paper: k = 26); 0 skips it")
     args = ap.parse_args(argv)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                       # timing rule: at least 3 warm-up steps
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return relaunch_with_ranks(args, argv)
+    if args.plumbing_only:
+        return run_plumbing_only(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

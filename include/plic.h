@@ -46,8 +46,10 @@ typedef struct CUstream_st *cudaStream_t;
                                   and to reproduce its defect: NaN for n = (1,0,0), V0 in {0,1}
                                   (PAPER.md:217, 256).  Not edge-case complete, not accurate for
                                   small normal components; no PLIC_FAST form.  Use PLIC_METHOD_SZ. */
-#define PLIC_METHOD_BLANK 0x40 /* plic_roundtrip_error only: the "blank run" of eq. (33), d0 = V0 - 1/2
-                                  in place of a PLIC solve */
+#define PLIC_METHOD_BLANK 0x40 /* the "blank run" of eq. (33): d0 = V0 - 1/2 in place of a PLIC solve
+                                  (PAPER.md:241-246).  In plic_roundtrip_error it is the run whose time
+                                  the paper subtracts; in plic_solve it is the same 4-read / 1-write
+                                  stream with no arithmetic, i.e. the ceiling of the access pattern */
 #define PLIC_FAST        0x100 /* approximate SFU roots/reciprocals/trig, branch-free a-priori
                                   case selection, two cells per packed fp32x2 instruction;
                                   without it: IEEE division and square root, CUDA libm
@@ -56,7 +58,8 @@ typedef struct CUstream_st *cudaStream_t;
 /* ---- error codes (functions return 0 on success, never throw, never print) ---------------- */
 #define PLIC_OK               0
 #define PLIC_ERR_NULL        -1 /* a null pointer with N > 0 */
-#define PLIC_ERR_SIZE        -2 /* N < 0 */
+#define PLIC_ERR_SIZE        -2 /* a size argument is out of range: N < 0, L < 2, work_entries < 2,
+                                   negative lattice extents or more than 2^31-1 lattice cells */
 #define PLIC_ERR_METHOD      -3 /* unknown method id */
 #define PLIC_ERR_LAUNCH      -4 /* the CUDA runtime reported an error (launch, copy, alloc) */
 #define PLIC_ERR_ALIGN       -5 /* a pointer is not 4-byte aligned */
@@ -197,6 +200,21 @@ const char *plic_error_string(int code);
 /* ABI version: 100*major + minor (1.04: + plic_roundtrip_error, plic_sphere_*, plic_curvature,
  * PLIC_METHOD_KAWANO). */
 int plic_version(void);
+
+/*
+ * plic_pipe_probe -- measurement support for the roofline denominators ("the
+ * builder must confirm [the per-SM rates] with an FFMA-only and a MUFU-only microbenchmark").
+ * Enqueues one launch of a kernel that executes a single kind of instruction in independent
+ * dependency chains (16 warps per SM sub-partition, SM count x 8 blocks of 256 threads) and
+ * stores in *warp_instructions (HOST pointer) how many warp-instructions of that kind the launch
+ * executes; the caller times the launch (CUDA events) and divides.
+ *   pipe  0 scalar FFMA, 1 packed FFMA2, 2 MUFU (rsqrt), 3 FMNMX (ALU pipe), 4 LOP3 (ALU pipe),
+ *         5 the halving step of nested-fast (2 FFMA2 + 2 LOP3 + FADD2 per pair)
+ *   trips loop trips per thread, >= 0 (64 instructions per chain set and trip; 320 for pipe 5)
+ *   sink  DEVICE pointer to >= 256 floats (never written in practice; keeps the chains alive)
+ * Returns PLIC_OK or PLIC_ERR_METHOD (unknown pipe) / _SIZE / _NULL / _LAUNCH.
+ */
+int plic_pipe_probe(int pipe, int trips, float *sink, int64_t *warp_instructions, cudaStream_t stream);
 
 /*
  * plic_launch_config -- the launch geometry plic_solve (method >= 0) or plic_volume

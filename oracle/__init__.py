@@ -11,6 +11,10 @@ lives entirely in the C file, whose header cites the paper passages it follows
     solve(V0, nx, ny, nz)  -> d0      bisection of the forward map on [-S/2, S/2]
     case(d0, nx, ny, nz)   -> 1..5    intersection case of eq. (11)
 
+``oracle.stratified`` (``stratified.c``) generates the case-stratified workload of BASELINE.json
+configs[2], which by its definition needs the case classifier and the forward map above; it is an
+input generator for tests and for bench.py's divergence leg, not part of the oracle's arithmetic.
+
 Sub-modules (numpy fp64, same rules): ``oracle.sphere`` -- the plane-sphere problem of sect. 3
 (eq. (37) and its inverse by bisection); ``oracle.curvature`` -- the curvature calculation of
 sect. 4 / appendix B (PY normal, PLIC point neighbourhood, paraboloid fit, eq. (63)).
@@ -25,16 +29,18 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "plic_oracle.c")
+_SRC_STRAT = os.path.join(_HERE, "stratified.c")    # configs[2] workload generator (inputs, not the oracle)
 _LIB = os.path.join(_HERE, "libplic_oracle.so")
 _lib = None
 
 
 def build(force: bool = False) -> str:
     """Compile plic_oracle.c with gcc (-O2, no fast-math, OpenMP) next to the source."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC),
+                                                                         os.path.getmtime(_SRC_STRAT)):
         tmp = _LIB + ".tmp.%d" % os.getpid()
         cmd = ["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
-               "-o", tmp, _SRC, "-lm"]
+               "-o", tmp, _SRC, _SRC_STRAT, "-lm"]
         subprocess.run(cmd, check=True)
         os.replace(tmp, _LIB)
     return _LIB
@@ -56,7 +62,7 @@ def _load():
         lib.oracle_plic_case.restype = i32
         lib.oracle_plic_volume_batch.argtypes = [dp, dp, dp, dp, dp, i64, i32]
         lib.oracle_plic_solve_batch.argtypes = [dp, dp, dp, dp, dp, i64, i32]
-        lib.oracle_plic_case_batch.argtypes = [dp, dp, dp, dp, ip, i64]
+        lib.oracle_plic_case_batch.argtypes = [dp, dp, dp, dp, ip, i64, i32]
         lib.oracle_plic_volume_batch_f32.argtypes = [fp, fp, fp, fp, dp, i64, i32]
         lib.oracle_plic_solve_batch_f32.argtypes = [fp, fp, fp, fp, dp, i64, i32]
         lib.oracle_max_threads.restype = i32
@@ -115,7 +121,7 @@ def solve(V0, nx, ny, nz, threads: int = 0) -> np.ndarray:
     return out.reshape(shape)
 
 
-def case(d0, nx, ny, nz) -> np.ndarray:
+def case(d0, nx, ny, nz, threads: int = 0) -> np.ndarray:
     """Intersection case 1..5 of eq. (11) for the plane (d0, n); 0 for the zero normal."""
     lib = _load()
     arrs = [np.asarray(a, dtype=np.float64) for a in (d0, nx, ny, nz)]
@@ -123,5 +129,5 @@ def case(d0, nx, ny, nz) -> np.ndarray:
     a, b, c, d = [np.ascontiguousarray(np.broadcast_to(x, shape)).ravel() for x in arrs]
     out = np.empty(a.shape[0], dtype=np.int32)
     lib.oracle_plic_case_batch(*[_ptr(x, ctypes.c_double) for x in (a, b, c, d)],
-                               _ptr(out, ctypes.c_int32), a.shape[0])
+                               _ptr(out, ctypes.c_int32), a.shape[0], threads)
     return out.reshape(shape)

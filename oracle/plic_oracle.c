@@ -173,9 +173,15 @@ void oracle_plic_solve_batch(const double *V0, const double *nx, const double *n
 }
 
 void oracle_plic_case_batch(const double *d0, const double *nx, const double *ny,
-                            const double *nz, int32_t *kase, int64_t N)
+                            const double *nz, int32_t *kase, int64_t N, int threads)
 {
     int64_t i;
+#ifdef _OPENMP
+    if (threads > 0) omp_set_num_threads(threads);
+#else
+    (void)threads;
+#endif
+#pragma omp parallel for schedule(static)
     for (i = 0; i < N; ++i) kase[i] = oracle_plic_case(d0[i], nx[i], ny[i], nz[i]);
 }
 

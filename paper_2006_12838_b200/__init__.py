@@ -28,7 +28,7 @@ __all__ = ["METHODS", "FAST", "BLANK", "KAWANO", "method_id", "plic_solve", "pli
            "plic_roundtrip_error", "plic_sphere_solve", "plic_sphere_volume", "plic_curvature",
            "plic_solve_host",
            "plic_volume_host", "plic_host_release", "plic_method_name", "plic_error_string",
-           "plic_version", "plic_launch_config", "plic_launch_count", "PlicError", "lib",
+           "plic_version", "plic_launch_config", "plic_pipe_probe", "PROBES", "plic_launch_count", "PlicError", "lib",
            "LIB_PATH"]
 
 METHODS = {"analytic": 0, "sz": 1, "newton": 2, "nested": 3}
@@ -78,6 +78,8 @@ def _load() -> ctypes.CDLL:
     lib_.plic_version.restype = ctypes.c_int
     lib_.plic_launch_config.argtypes = [ctypes.c_int, i64, ip, ip, ip]
     lib_.plic_launch_config.restype = ctypes.c_int
+    lib_.plic_pipe_probe.argtypes = [ctypes.c_int, ctypes.c_int, fp, ctypes.POINTER(i64), ctypes.c_void_p]
+    lib_.plic_pipe_probe.restype = ctypes.c_int
     lib_.plic_launch_count.argtypes = []
     lib_.plic_launch_count.restype = i64
     return lib_
@@ -131,6 +133,23 @@ def plic_launch_config(method, N: int, fast: bool = False):
     if rc != 0:
         raise PlicError(rc, "plic_launch_config")
     return g.value, b.value, c.value
+
+
+PROBES = {"ffma": 0, "ffma2": 1, "mufu": 2, "fmnmx": 3, "lop3": 4, "nested_step": 5, "ffma+lop3": 6,
+          "ffma2+lop3": 7, "mufu+4ffma": 8, "ffma+fmnmx": 9, "fsetp+fsel": 10, "nested_step_scalar": 11,
+          "nested_step_hybrid": 12, "fadd": 13, "fmul": 14, "fadd2": 15, "2ffma+lop3+fadd": 16}
+
+
+def plic_pipe_probe(pipe, trips: int, sink, stream=None) -> int:
+    """Enqueues one instruction-rate probe launch (include/plic.h); returns the number of
+    warp-instructions of the probed kind that launch executes.  `sink`: float32 CUDA tensor, >= 256."""
+    n = i64_out = ctypes.c_int64(0)
+    pid = PROBES[pipe] if isinstance(pipe, str) else int(pipe)
+    rc = lib.plic_pipe_probe(pid, int(trips), sink.data_ptr(), ctypes.byref(i64_out),
+                             _stream_handle(stream, sink.device))
+    if rc != 0:
+        raise PlicError(rc, "plic_pipe_probe")
+    return int(n.value)
 
 
 def plic_host_release() -> None:

@@ -26,6 +26,7 @@
 #include "plic_methods.cuh"
 #include "plic_packed.cuh"
 #include "plic_curvature.cuh"
+#include "plic_probe.cuh"
 
 #define PLIC_VERSION 104
 
@@ -114,6 +115,20 @@ struct VolumeOp {
         const F2 lo = volume_pair(F2{v.x, v.y}, F2{a.x, a.y}, F2{b.x, b.y}, F2{c.x, c.y});
         const F2 hi = volume_pair(F2{v.z, v.w}, F2{a.z, a.w}, F2{b.z, b.w}, F2{c.z, c.w});
         return make_float4(lo.x, lo.y, hi.x, hi.y);
+    }
+};
+
+// The "blank run" of eq. (33) as a map: d0 = V0 - 1/2, with the same four input streams and the
+// same body kernel (map_tma) as the HBM-bound solvers, i.e. the ceiling of this access pattern
+// (4 arrays read, 1 written) for bench.py's stream_ceiling.  The bulk copies bring all four
+// tiles into shared memory whether or not the threads read them.
+struct BlankOp {
+    static constexpr int kBody = BODY_TMA;
+    static constexpr int kMinBlocks = 5;
+    static __device__ __forceinline__ float apply(float s, float, float, float) { return s - 0.5f; }
+    static __device__ __forceinline__ float4 apply4(const float4 &v, const float4 &, const float4 &,
+                                                    const float4 &) {
+        return make_float4(v.x - 0.5f, v.y - 0.5f, v.z - 0.5f, v.w - 0.5f);
     }
 };
 
@@ -386,6 +401,7 @@ static BodyKernel vec_kernel(int k) {
         case 6: return body_of<SolveOp<NEWTON, true>>();
         case 7: return body_of<SolveOp<NESTED, true>>();
         case 9: return body_of<SolveOp<KAWANO, false>>();
+        case 10: return body_of<BlankOp>();
         default: return body_of<VolumeOp>();
     }
 }
@@ -400,6 +416,7 @@ static scalar_kernel_t scalar_kernel(int k) {
         case 6: return map_scalar<SolveOp<NEWTON, true>>;
         case 7: return map_scalar<SolveOp<NESTED, true>>;
         case 9: return map_scalar<SolveOp<KAWANO, false>>;
+        case 10: return map_scalar<BlankOp>;
         default: return map_scalar<VolumeOp>;
     }
 }
@@ -407,6 +424,7 @@ static scalar_kernel_t scalar_kernel(int k) {
 // kernel index for a method id; -1 if the id is unknown
 static int kernel_index(int method) {
     if (method == PLIC_METHOD_KAWANO) return 2 * PLIC_NUM_METHODS + 1;     // precise only
+    if (method == PLIC_METHOD_BLANK) return 2 * PLIC_NUM_METHODS + 2;      // d0 = V0 - 1/2
     const int base = method & ~PLIC_FAST;
     if (base < 0 || base >= PLIC_NUM_METHODS) return -1;
     return base + ((method & PLIC_FAST) ? PLIC_NUM_METHODS : 0);
@@ -448,10 +466,6 @@ static int launch_map(int k, const float *s, const float *nx, const float *ny, c
         if (ps[i] & 3u) return PLIC_ERR_ALIGN;
         if ((ps[i] & 15u) != (ps[0] & 15u)) same = false;
     }
-    cudaError_t err;
-    const DeviceInfo *info = device_info(&err);
-    if (!info) return PLIC_ERR_LAUNCH;
-
     // cells before the first 16-byte boundary, then n4 full float4 groups, then the tail
     int64_t head = same ? (int64_t)(((16u - (ps[0] & 15u)) & 15u) >> 2) : N;
     if (head > N) head = N;
@@ -484,7 +498,7 @@ static int launch_map(int k, const float *s, const float *nx, const float *ny, c
                                                                       tail0, N);
         g_launches.fetch_add(1, std::memory_order_relaxed);
     }
-    return cudaGetLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
+    return cudaPeekAtLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -624,7 +638,7 @@ static int launch_map1(const float *in, float *out, int64_t N, cudaStream_t stre
                                                                                  tail0, N);
         g_launches.fetch_add(1, std::memory_order_relaxed);
     }
-    return cudaGetLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
+    return cudaPeekAtLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -720,21 +734,17 @@ int plic_volume(const float *d0, const float *nx, const float *ny, const float *
 
 int plic_roundtrip_error(const float *nx, const float *ny, const float *nz, float *E, int64_t N,
                          int L, int method, cudaStream_t stream) {
-    const int k = method == PLIC_METHOD_BLANK ? plic::kVolumeKernel : plic::kernel_index(method);
+    const int k = method == PLIC_METHOD_BLANK ? plic::kVolumeKernel : plic::kernel_index(method);   // blank: default case
     if (k < 0) return PLIC_ERR_METHOD;
     if (N < 0 || L < 2) return PLIC_ERR_SIZE;
     if (N == 0) return PLIC_OK;
     if (!nx || !ny || !nz || !E) return PLIC_ERR_NULL;
     if (((uintptr_t)nx | (uintptr_t)ny | (uintptr_t)nz | (uintptr_t)E) & 3u) return PLIC_ERR_ALIGN;
-    cudaError_t err;
-    const plic::DeviceInfo *info = plic::device_info(&err);
-    if (!info) return PLIC_ERR_LAUNCH;
     // compute bound: one thread per normal, one block per 256 normals (hardware block scheduling)
-    (void)info;
     plic::roundtrip_kernel_of(k)<<<plic::grid_for(N, 1), plic::kBlock, 0, stream>>>(
         nx, ny, nz, E, N, L);
     plic::g_launches.fetch_add(1, std::memory_order_relaxed);
-    return cudaGetLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
+    return cudaPeekAtLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
 }
 
 int plic_sphere_solve(const float *V0, float *d0, int64_t N, int fast, cudaStream_t stream) {
@@ -791,7 +801,7 @@ int plic_curvature(const float *phi, float *kappa, int nx, int ny, int nz, int32
             return PLIC_ERR_LAUNCH;
     }
     plic::g_launches.fetch_add(2, std::memory_order_relaxed);
-    return cudaGetLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
+    return cudaPeekAtLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
 }
 
 int plic_solve_host(const float *V0, const float *nx, const float *ny, const float *nz,
@@ -832,7 +842,7 @@ const char *plic_error_string(int code) {
     switch (code) {
         case PLIC_OK: return "ok";
         case PLIC_ERR_NULL: return "null pointer with N > 0";
-        case PLIC_ERR_SIZE: return "negative N";
+        case PLIC_ERR_SIZE: return "size argument out of range";
         case PLIC_ERR_METHOD: return "unknown method id";
         case PLIC_ERR_LAUNCH: return "CUDA runtime error";
         case PLIC_ERR_ALIGN: return "pointer not 4-byte aligned";
@@ -841,6 +851,52 @@ const char *plic_error_string(int code) {
 }
 
 int plic_version(void) { return PLIC_VERSION; }
+
+int plic_pipe_probe(int pipe, int trips, float *sink, int64_t *warp_instructions, cudaStream_t stream) {
+    if (pipe < 0 || pipe >= plic::PROBE_COUNT) return PLIC_ERR_METHOD;
+    if (trips < 0) return PLIC_ERR_SIZE;
+    if (!sink || !warp_instructions) return PLIC_ERR_NULL;
+    cudaError_t err;
+    const plic::DeviceInfo *info = plic::device_info(&err);
+    if (!info) return PLIC_ERR_LAUNCH;
+    const int grid = info->sms * plic::kProbeBlocksPerSm;
+    const int64_t warps = (int64_t)grid * (plic::kBlock / 32);
+    int64_t per_trip = 0;
+#define PLIC_PROBE_CASE(P) \
+    case plic::P: plic::pipe_probe<plic::P><<<grid, plic::kBlock, 0, stream>>>(sink, trips); \
+                  per_trip = (int64_t)plic::kProbeChains * plic::kProbeUnroll * plic::ProbeOp<plic::P>::kInst; break;
+    switch (pipe) {
+        PLIC_PROBE_CASE(PROBE_FFMA)
+        PLIC_PROBE_CASE(PROBE_FFMA2)
+        PLIC_PROBE_CASE(PROBE_MUFU)
+        PLIC_PROBE_CASE(PROBE_FMNMX)
+        PLIC_PROBE_CASE(PROBE_LOP3)
+        PLIC_PROBE_CASE(PROBE_FFMA_LOP3)
+        PLIC_PROBE_CASE(PROBE_FFMA2_LOP3)
+        PLIC_PROBE_CASE(PROBE_MUFU_FFMA4)
+        PLIC_PROBE_CASE(PROBE_FFMA_FMNMX)
+        PLIC_PROBE_CASE(PROBE_FSEL)
+        PLIC_PROBE_CASE(PROBE_FADD)
+        PLIC_PROBE_CASE(PROBE_FMUL)
+        PLIC_PROBE_CASE(PROBE_FADD2)
+        PLIC_PROBE_CASE(PROBE_3FP_LOP3)
+        case plic::PROBE_NESTED_SCALAR:
+            plic::pipe_probe_nested_alt<0><<<grid, plic::kBlock, 0, stream>>>(sink, trips);
+            per_trip = 4 * 16 * 8;                               // 4 pairs x 16 halvings x 8 instructions
+            break;
+        case plic::PROBE_NESTED_HYBRID:
+            plic::pipe_probe_nested_alt<1><<<grid, plic::kBlock, 0, stream>>>(sink, trips);
+            per_trip = 4 * 16 * 6;
+            break;
+        default:
+            plic::pipe_probe_nested<<<grid, plic::kBlock, 0, stream>>>(sink, trips);
+            per_trip = 4 * 16 * 5;                               // 4 pairs x 16 halvings x 5 instructions
+    }
+#undef PLIC_PROBE_CASE
+    *warp_instructions = warps * per_trip * trips;
+    plic::g_launches.fetch_add(1, std::memory_order_relaxed);
+    return cudaPeekAtLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
+}
 
 int plic_launch_config(int method, int64_t N, int *grid, int *block, int *cells_per_thread) {
     const int k = method == -1 ? plic::kVolumeKernel : plic::kernel_index(method);

@@ -310,6 +310,11 @@ struct PairSolver<NEWTON> {
 // immediate slot is free for the step size (as a literal mask, ptxas moves every step constant
 // into a register first: one more instruction per step).
 __constant__ unsigned kSignMask = 0x80000000u;
+__device__ __forceinline__ unsigned sign_mask_register() {
+    unsigned m;
+    asm volatile("{ .reg .u64 a; cvta.to.const.u64 a, %1; ld.const.u32 %0, [a]; }" : "=r"(m) : "l"(&kSignMask));
+    return m;
+}
 
 template <unsigned STEP_BITS>
 __device__ __forceinline__ float signed_step(float G, unsigned mask) {
@@ -359,7 +364,7 @@ struct PairSolver<NESTED> {
         const F2 nP = mul2(np, iw2);                                            // -p / w^2
         const F2 nR = mul2(mul2(nr, iw), iw2);                                  // -r / w^3
         F2 c = fma2(lo, iw, f2(0.5f));
-        NestedSteps<0, 20>::run(c, nP, nR, kSignMask);
+        NestedSteps<0, 20>::run(c, nP, nR, sign_mask_register());
         const F2 d34 = max2(fma2(c, w, sel2(c4, in.hS, n12)), n2);              // floor; drops NaN
         d = sel2(gt2(t1, mul2(n2, sub2(n2, n1))), d34, d);
         return sel2(le2(n12, W), mul2(add2(W, n12), 0.5f), d);                  // (5)

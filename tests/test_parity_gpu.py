@@ -16,8 +16,7 @@ import torch
 import gen
 import oracle
 
-sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
-from stratified import stratified  # noqa: E402
+from oracle.stratified import stratified
 
 pytestmark = pytest.mark.gpu
 
