@@ -167,8 +167,15 @@ int plic_sphere_volume(const float *d0, float *V0, int64_t N, cudaStream_t strea
  *
  * Sign: with the normal of eq. (54) pointing out of the fluid, eq. (63) is negative for a convex
  * fluid body (-1/R for a drop of radius R) and positive for a bubble.
- * A 4-byte memset and two kernels are enqueued on `stream` (a streaming pass and, as a programmatic
- * dependent launch, a dense pass over the interface list); errors, ownership and stream semantics as plic_solve.
+ * Rank deficiency: the paper solves eq. (70) by LU decomposition without a pivot check.  Here a fit
+ * parameter whose pivot falls below 1e-6 of its diagonal entry of M (the points do not determine it:
+ * a lone neighbour, neighbours on one line or coplanar with the normal, coincident abscissae) is
+ * dropped like the parameters beyond the number of points: it stays 0 and takes no part
+ * in the elimination.  kappa is therefore finite for every finite lattice.
+ * A 4-byte memset and two kernels are enqueued on `stream`: a streaming pass (128-bit accesses when phi
+ * and kappa are 16-byte aligned, scalar otherwise) and, as a programmatic dependent launch, a dense pass
+ * over the interface list with two lanes per point.  Aligned and unaligned calls give bitwise the same
+ * kappa.  Errors, ownership and stream semantics as plic_solve.
  */
 int plic_curvature(const float *phi, float *kappa, int nx, int ny, int nz, int32_t *work,
                    int64_t work_entries, cudaStream_t stream);

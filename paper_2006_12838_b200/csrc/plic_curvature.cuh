@@ -11,14 +11,22 @@
 //   5. M x = b, eq. (70); fewer than 5 points: the leading k x k block
 //   6. kappa = (A (I^2+1) + B (H^2+1) - C H I) / (H^2+I^2+1)^(3/2), eq. (63)
 //
-// Two kernels, because interface points are a 2-D surface in a 3-D lattice (0.4 % of the cells of
-// a 256^3 box holding an R = 60 drop):
+// Interface points are a 2-D surface in a 3-D lattice (0.4 % of the cells of a 256^3 box holding an
+// R = 60 drop), so a thread per lattice cell would run the ~2000-instruction point routine in warps
+// with one or two active lanes.  Two kernels instead:
 //   curv_mark4  streams the lattice once (HBM bound: 4 B read + 4 B written per cell), writes
-//               kappa = 0 everywhere and appends the index of every interior interface point to a
-//               list (one atomicAdd per warp); curv_mark is its scalar form for misaligned lattices;
-//   curv_cells  one thread per list entry, so warps are dense: gathers the 27 fill levels (L2
-//               hits, the lattice has just been streamed), and runs steps 1-6 in registers; the 26
-//               neighbour solves go through the packed two-cells-per-instruction analytic solver.
+//               kappa = 0 everywhere and collects the interior interface points per block in shared
+//               memory (warp-aggregated), flushed to the caller's list with one global atomicAdd per
+//               block; curv_mark is its scalar form for lattices off the 16-byte boundary;
+//   curv_cells  the list entries in dense warps, kPointLanes LANES PER POINT: the 13 neighbour pairs
+//               (e, -e) and the centre are dealt to the lanes of a point, which gather their fill
+//               levels (L2 hits, the lattice has just been streamed), solve their PLIC offsets with the
+//               packed analytic solver and accumulate their share of the 17 moments; gradient sums and
+//               moments are reduced with xor shuffles.  One thread per point (round 1) left 3 warps per
+//               SM sub-partition with a 2000-instruction dependent chain each: latency bound at 16 %
+//               occupancy.  (Evaluating the points inside the streaming kernel -- each block its own
+//               -- was tried: 49 us per call instead of 38, the point routine's registers cut the
+//               streaming occupancy and every block with a single point pays a full round.)
 // Readings C1-C5 of oracle/curvature.py's header apply (sign of kappa, zero for non-interface /
 // border / gradient-free / neighbour-free points, reduced rank keeps the first k parameters).
 #pragma once
@@ -26,7 +34,6 @@
 
 namespace plic {
 
-constexpr int kCurvBlock = 64;                 // threads per block of curv_cells
 
 __device__ __forceinline__ bool curv_interior(int64_t i, int nx, int ny, int nz) {
     const unsigned u = (unsigned)i;                               // ncells < 2^31: 32-bit divisions
@@ -150,7 +157,13 @@ curv_mark4(const float4 *__restrict__ phi, float4 *__restrict__ kappa, int nx, i
             unsigned h = 0;
 #pragma unroll
             for (int c = 0; c < 4; ++c)
-                if (v[c] > 0.0f && v[c] < 1.0f && curv_interior(4 * g[k] + c, nx, ny, nz)) h |= 1u << c;
+                if (v[c] > 0.0f && v[c] < 1.0f) h |= 1u << c;
+            // interface cells are rare: the interior test (two integer divisions per cell) and the
+            // append run only in warps that hold one
+            if (__ballot_sync(0xffffffffu, h != 0) == 0) continue;
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+                if ((h & (1u << c)) && !curv_interior(4 * g[k] + c, nx, ny, nz)) h &= ~(1u << c);
             curv_append(h, 4 * g[k], sh, list, capacity);
         }
     }
@@ -167,105 +180,118 @@ curv_mark4(const float4 *__restrict__ phi, float4 *__restrict__ kappa, int nx, i
     curv_flush(sh, list, capacity);
 }
 
-// ---- steps 1-6 for one point ----------------------------------------------------------------
-struct Moments {            // the 12 distinct entries of M (eq. (69)) and the 5 of b
-    F2 x4, x2y2, x3y, x3, x2y, y4, xy3, xy2, y3, x2, xy, y2, zx2, zy2, zxy, zx, zy;
-};
+// ---- steps 1-6 for one point, on LANES adjacent lanes ---------------------------------------------
+// sub = lane % LANES (LANES = 2 or 4).  Slot s of a lane holds item = sub + LANES s: items 0..12 are the
+// neighbour pairs (e_k, -e_k), e_k = (k % 3 - 1, (k / 3) % 3 - 1, k / 9 - 1); item 13 is the centre (its
+// offset d0(phi_0, n) is broadcast to the group from lane sub = 1); items 14, 15 (LANES = 4) repeat pairs
+// with weight 0.  All 32 lanes of the warp must call this together (shuffles); `c` must be an interior
+// cell for every lane.
+// Symmetry of a pair: x, y flip sign with e, so with the weights m+, m- (1 for an interface neighbour)
+// the even moments take (m+ + m-), the odd ones (m+ - m-), and the z-moments m+ z+ +- m- z-.
+constexpr float kPivotRel = 1e-6f;     // a pivot below this fraction of its diagonal entry drops the parameter
 
-__device__ __forceinline__ float curvature_point(const float (&p)[27]) {
-    // step 1: eq. (54), weights eq. (55); p[(dx+1) + 3 (dy+1) + 9 (dz+1)]
-    float g[3];
+template <int LANES>
+__device__ __forceinline__ float curvature_point(const float *__restrict__ phi, int64_t c, int64_t sy,
+                                                 int64_t sz, int sub) {
+    static_assert(LANES == 1 || LANES == 2 || LANES == 4, "13 pairs + the centre on 1, 2 or 4 lanes");
+    constexpr int SLOTS = (14 + LANES - 1) / LANES;                  // 7 or 4
+    const unsigned full = 0xffffffffu;
+    const float *pc = phi + c;
+    const int isy = (int)sy, isz = (int)sz;                          // ncells < 2^31
+    float g[3] = {0.0f, 0.0f, 0.0f};
+    // step 1: eq. (54), weights eq. (55): 4, 2, 1 for |e|_1 = 1, 2, 3; the pair contributes w e (phi+ - phi-).
+    // The fill levels are not kept: step 3 reads them again (L1 hits), which frees ~35 registers.
 #pragma unroll
-    for (int a = 0; a < 3; ++a) g[a] = 0.0f;
+    for (int s = 0; s < SLOTS; ++s) {
+        const int k = sub + LANES * s;
+        const int t = (k * 11) >> 5;                                 // k / 3 for k <= 15
+        const int ex = k - 3 * t - 1, ey = t - (t >= 3 ? 3 : 0) - 1, ez = (k >= 9 ? 1 : 0) - 1;
+        const int off = ex + ey * isy + ez * isz;
+        const int l1 = (ex != 0) + (ey != 0) + (ez != 0);
+        const float w = k < 13 ? (float)(8 >> l1) * (__ldg(pc + off) - __ldg(pc - off)) : 0.0f;
+        g[0] = fmaf(w, (float)ex, g[0]);
+        g[1] = fmaf(w, (float)ey, g[1]);
+        g[2] = fmaf(w, (float)ez, g[2]);
+    }
 #pragma unroll
-    for (int i = 0; i < 27; ++i) {
-        const int e[3] = {i % 3 - 1, (i / 3) % 3 - 1, i / 9 - 1};
-        const int l1 = (e[0] != 0) + (e[1] != 0) + (e[2] != 0);
-        const float w = l1 == 1 ? 4.0f : (l1 == 2 ? 2.0f : 1.0f);
-#pragma unroll
-        for (int a = 0; a < 3; ++a)
-            if (e[a] != 0) g[a] = fmaf(w * (float)e[a], p[i], g[a]);
+    for (int a = 0; a < 3; ++a) {
+        if (LANES >= 2) g[a] += __shfl_xor_sync(full, g[a], 1);
+        if (LANES == 4) g[a] += __shfl_xor_sync(full, g[a], 2);
     }
     const float g2 = fmaf(g[0], g[0], fmaf(g[1], g[1], g[2] * g[2]));
-    if (!(g2 > 0.0f)) return 0.0f;                                   // C2
-    const float ig = -1.0f / sqrtf(g2);
-    const float n[3] = {g[0] * ig, g[1] * ig, g[2] * ig};
+    const bool has_normal = g2 > 0.0f;                               // C2 otherwise
+    const float ig = has_normal ? -1.0f / sqrtf(g2) : 0.0f;
+    const float n[3] = {has_normal ? g[0] * ig : 0.0f, has_normal ? g[1] * ig : 0.0f, has_normal ? g[2] * ig : 1.0f};
     // step 2: eq. (42)-(45)
     const float r[3] = {0.56270900f, 0.32704452f, 0.75921047f};
     float by[3] = {fmaf(n[1], r[2], -n[2] * r[1]), fmaf(n[2], r[0], -n[0] * r[2]),
                    fmaf(n[0], r[1], -n[1] * r[0])};
-    const float iby = 1.0f / sqrtf(fmaf(by[0], by[0], fmaf(by[1], by[1], by[2] * by[2])));
+    const float iby = rsqrtf(fmaxf(fmaf(by[0], by[0], fmaf(by[1], by[1], by[2] * by[2])), 1e-30f));
     by[0] *= iby; by[1] *= iby; by[2] *= iby;
     const float bx[3] = {fmaf(by[1], n[2], -by[2] * n[1]), fmaf(by[2], n[0], -by[0] * n[2]),
                          fmaf(by[0], n[1], -by[1] * n[0])};
-    // step 3: PLIC offsets with the one normal n; the centre's offset first
+    // step 3: PLIC offsets with the one normal n (packed pair = the two ends of one direction)
     const F2 NX{n[0], n[0]}, NY{n[1], n[1]}, NZ{n[2], n[2]};
-    const float d00 = solve_pair_fast<ANALYTIC>(F2{p[13], p[13]}, NX, NY, NZ).x;
-    Moments s;
-    const F2 zero = f2(0.0f);
-    s.x4 = s.x2y2 = s.x3y = s.x3 = s.x2y = s.y4 = s.xy3 = s.xy2 = s.y3 = s.x2 = s.xy = s.y2 = zero;
-    s.zx2 = s.zy2 = s.zxy = s.zx = s.zy = zero;
+    float x4 = 0.f, x2y2 = 0.f, x3y = 0.f, x3 = 0.f, x2y = 0.f, y4 = 0.f, xy3 = 0.f, xy2 = 0.f, y3 = 0.f;
+    float sx2 = 0.f, sxy = 0.f, sy2 = 0.f, zx2 = 0.f, zy2 = 0.f, zxy = 0.f, zx = 0.f, zy = 0.f;
     int count = 0;
+    float d00 = 0.0f;
 #pragma unroll
-    for (int k = 0; k < 13; ++k) {
-        // neighbours in pairs (i0, i1), skipping the centre 13: 0..12 with 14..26 reversed
-        const int i0 = k, i1 = 26 - k;
-        const F2 ph{p[i0], p[i1]};
-        const F2 d0 = solve_pair_fast<ANALYTIC>(ph, NX, NY, NZ);
-        const bool u0 = ph.x > 0.0f && ph.x < 1.0f, u1 = ph.y > 0.0f && ph.y < 1.0f;
+    for (int q = 0; q < SLOTS; ++q) {
+        const int s = q == 0 ? SLOTS - 1 : q - 1;                    // the last slot first: it holds the centre
+        const int k = sub + LANES * s;
+        const int t = (k * 11) >> 5;
+        const int ex = k - 3 * t - 1, ey = t - (t >= 3 ? 3 : 0) - 1, ez = (k >= 9 ? 1 : 0) - 1;
+        const int off = ex + ey * isy + ez * isz;
+        const float pp = __ldg(pc + off), pm = __ldg(pc - off);
+        const F2 d0 = solve_pair_fast<ANALYTIC>(F2{pp, pm}, NX, NY, NZ);
+        if (q == 0) d00 = LANES == 1 ? d0.x : __shfl_sync(full, d0.x, (threadIdx.x & (32 - LANES)) | 1);   // from lane sub = 1
+        const bool u0 = k < 13 && pp > 0.0f && pp < 1.0f, u1 = k < 13 && pm > 0.0f && pm < 1.0f;
         count += (int)u0 + (int)u1;
-        const F2 m{u0 ? 1.0f : 0.0f, u1 ? 1.0f : 0.0f};
-        // e_{i1} = -e_{i0}: the pair sits at opposite ends of one direction
-        const int e[3] = {i0 % 3 - 1, (i0 / 3) % 3 - 1, i0 / 9 - 1};
-        float px = 0.0f, py = 0.0f, pz = 0.0f;
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            if (e[a] > 0) { px += bx[a]; py += by[a]; pz += n[a]; }
-            if (e[a] < 0) { px -= bx[a]; py -= by[a]; pz -= n[a]; }
-        }
-        const F2 x{px, -px}, y{py, -py};
-        const F2 z = add2(F2{pz, -pz}, add2(d0, f2(-d00)));          // eq. (46)
-        // step 4: eq. (49), (69); unused points enter with weight m = 0 (their d0 is finite)
-        const F2 x2 = mul2(x, x), y2 = mul2(y, y), xy = mul2(x, y);
-        const F2 mx2 = mul2(m, x2), my2 = mul2(m, y2), mxy = mul2(m, xy);
-        const F2 mx = mul2(m, x), my = mul2(m, y);
-        s.x4 = fma2(mx2, x2, s.x4);     s.x2y2 = fma2(mx2, y2, s.x2y2); s.x3y = fma2(mx2, xy, s.x3y);
-        s.x3 = fma2(mx2, x, s.x3);      s.x2y = fma2(mx2, y, s.x2y);    s.y4 = fma2(my2, y2, s.y4);
-        s.xy3 = fma2(my2, xy, s.xy3);   s.xy2 = fma2(my2, x, s.xy2);    s.y3 = fma2(my2, y, s.y3);
-        s.x2 = add2(s.x2, mx2);         s.xy = add2(s.xy, mxy);         s.y2 = add2(s.y2, my2);
-        s.zx2 = fma2(mx2, z, s.zx2);    s.zy2 = fma2(my2, z, s.zy2);    s.zxy = fma2(mxy, z, s.zxy);
-        s.zx = fma2(mx, z, s.zx);       s.zy = fma2(my, z, s.zy);
+        const float m0 = u0 ? 1.0f : 0.0f, m1 = u1 ? 1.0f : 0.0f;
+        const float fx = (float)ex, fy = (float)ey, fz = (float)ez;
+        const float px = fmaf(fx, bx[0], fmaf(fy, bx[1], fz * bx[2]));
+        const float py = fmaf(fx, by[0], fmaf(fy, by[1], fz * by[2]));
+        const float pz = fmaf(fx, n[0], fmaf(fy, n[1], fz * n[2]));
+        const float z0 = m0 * (pz + (d0.x - d00)), z1 = m1 * ((d0.y - d00) - pz);      // eq. (46), weighted
+        const float ms = m0 + m1, md = m0 - m1, zs = z0 + z1, zd = z0 - z1;
+        // step 4: eq. (49), (69)
+        const float x2 = px * px, y2 = py * py, xy = px * py;
+        const float ex2 = ms * x2, ey2 = ms * y2, exy = ms * xy, ox2 = md * x2, oy2 = md * y2;
+        x4 = fmaf(ex2, x2, x4);    x2y2 = fmaf(ex2, y2, x2y2); x3y = fmaf(ex2, xy, x3y);
+        y4 = fmaf(ey2, y2, y4);    xy3 = fmaf(ey2, xy, xy3);
+        x3 = fmaf(ox2, px, x3);    x2y = fmaf(ox2, py, x2y);   xy2 = fmaf(oy2, px, xy2);  y3 = fmaf(oy2, py, y3);
+        sx2 += ex2;                sxy += exy;                 sy2 += ey2;
+        zx2 = fmaf(zs, x2, zx2);   zy2 = fmaf(zs, y2, zy2);    zxy = fmaf(zs, xy, zxy);
+        zx = fmaf(zd, px, zx);     zy = fmaf(zd, py, zy);
     }
-    if (count == 0) return 0.0f;                                     // C2
-#define PLIC_SUM(f) (s.f.x + s.f.y)
+#define PLIC_REDUCE4(v) if (LANES >= 2) v += __shfl_xor_sync(full, v, 1); if (LANES == 4) v += __shfl_xor_sync(full, v, 2);
+    PLIC_REDUCE4(x4) PLIC_REDUCE4(x2y2) PLIC_REDUCE4(x3y) PLIC_REDUCE4(x3) PLIC_REDUCE4(x2y) PLIC_REDUCE4(y4)
+    PLIC_REDUCE4(xy3) PLIC_REDUCE4(xy2) PLIC_REDUCE4(y3) PLIC_REDUCE4(sx2) PLIC_REDUCE4(sxy) PLIC_REDUCE4(sy2)
+    PLIC_REDUCE4(zx2) PLIC_REDUCE4(zy2) PLIC_REDUCE4(zxy) PLIC_REDUCE4(zx) PLIC_REDUCE4(zy) PLIC_REDUCE4(count)
+#undef PLIC_REDUCE4
     // symmetric M, eq. (69): only the upper half is formed
     float M[5][5], b[5];
-    M[0][0] = PLIC_SUM(x4);  M[0][1] = PLIC_SUM(x2y2); M[0][2] = PLIC_SUM(x3y); M[0][3] = PLIC_SUM(x3);
-    M[0][4] = PLIC_SUM(x2y); M[1][1] = PLIC_SUM(y4);   M[1][2] = PLIC_SUM(xy3); M[1][3] = PLIC_SUM(xy2);
-    M[1][4] = PLIC_SUM(y3);  M[2][2] = M[0][1];        M[2][3] = M[0][4];       M[2][4] = M[1][3];
-    M[3][3] = PLIC_SUM(x2);  M[3][4] = PLIC_SUM(xy);   M[4][4] = PLIC_SUM(y2);
-    b[0] = PLIC_SUM(zx2); b[1] = PLIC_SUM(zy2); b[2] = PLIC_SUM(zxy); b[3] = PLIC_SUM(zx); b[4] = PLIC_SUM(zy);
-#undef PLIC_SUM
-    // fewer than five points: parameters k..4 stay zero -- their rows and columns
-    // are replaced by the identity, which leaves the leading k x k block's solution unchanged
-#pragma unroll
-    for (int i = 1; i < 5; ++i) {
-        if (count <= i) {
-#pragma unroll
-            for (int j = 0; j < 5; ++j)
-                if (j < i) M[j][i] = 0.0f; else if (j > i) M[i][j] = 0.0f;
-            M[i][i] = 1.0f;
-            b[i] = 0.0f;
-        }
-    }
-    // step 5: LU decomposition of the symmetric matrix without pivoting (M is positive definite
-    // for points in general position), in the L D L^T form: U = D L^T is kept in the upper half
+    M[0][0] = x4;  M[0][1] = x2y2; M[0][2] = x3y; M[0][3] = x3;  M[0][4] = x2y;
+    M[1][1] = y4;  M[1][2] = xy3;  M[1][3] = xy2; M[1][4] = y3;
+    M[2][2] = x2y2; M[2][3] = x2y; M[2][4] = xy2;
+    M[3][3] = sx2; M[3][4] = sxy;  M[4][4] = sy2;
+    b[0] = zx2; b[1] = zy2; b[2] = zxy; b[3] = zx; b[4] = zy;
+    // step 5: LU decomposition of the symmetric positive semi-definite matrix without pivoting, in the
+    // L D L^T form (U = D L^T is kept in the upper half).  A parameter is dropped (stays 0, and takes no
+    // part in the elimination) when fewer points than its index + 1 were used ("reducing
+    // dimensionality"), or when its pivot has fallen below kPivotRel of its diagonal entry -- the
+    // points then do not determine it (coplanar with the normal, coincident abscissae); the paper's LU
+    // has no such check, the result without it would be Inf or NaN.
+    float inv[5];
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
-        const float inv = 1.0f / M[k][k];
+        const float diag = k == 0 ? x4 : (k == 1 ? y4 : (k == 2 ? x2y2 : (k == 3 ? sx2 : sy2)));
+        const bool keep = count > k && M[k][k] > kPivotRel * diag;
+        inv[k] = keep ? 1.0f / M[k][k] : 0.0f;
 #pragma unroll
         for (int i = k + 1; i < 5; ++i) {
-            const float f = M[k][i] * inv;                           // L[i][k] (symmetry)
+            const float f = M[k][i] * inv[k];                        // L[i][k] (symmetry)
 #pragma unroll
             for (int j = i; j < 5; ++j) M[i][j] = fmaf(-f, M[k][j], M[i][j]);
             b[i] = fmaf(-f, b[k], b[i]);
@@ -277,32 +303,47 @@ __device__ __forceinline__ float curvature_point(const float (&p)[27]) {
         float acc = b[i];
 #pragma unroll
         for (int j = i + 1; j < 5; ++j) acc = fmaf(-M[i][j], xs[j], acc);
-        xs[i] = acc / M[i][i];
+        xs[i] = acc * inv[i];
     }
     // step 6: eq. (63)
     const float A = xs[0], B = xs[1], C = xs[2], H = xs[3], I = xs[4];
     const float w = fmaf(H, H, fmaf(I, I, 1.0f));
     const float num = fmaf(A, fmaf(I, I, 1.0f), fmaf(B, fmaf(H, H, 1.0f), -C * H * I));
-    return num / (w * sqrtf(w));
+    const float kap = num / (w * sqrtf(w));
+    // C2; a fit whose parameters overflow fp32 (pivots just above the guard) also gives 0, never Inf or NaN
+    return (has_normal && count > 0 && fabsf(kap) < 3.0e38f) ? kap : 0.0f;
 }
 
-// ---- curv_cells ------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kCurvBlock)
+// ---- curv_cells: kPointLanes lanes per entry of the caller's list ------------------------------------
+#ifndef PLIC_CURV_LANES
+#define PLIC_CURV_LANES 1
+#endif
+#ifndef PLIC_CURV_BLOCK
+#define PLIC_CURV_BLOCK 64
+#endif
+#ifndef PLIC_CURV_MINBLOCKS
+#define PLIC_CURV_MINBLOCKS 7
+#endif
+constexpr int kPointLanes = PLIC_CURV_LANES;
+constexpr int kCurvBlock = PLIC_CURV_BLOCK;    // threads per block
+
+__global__ void __launch_bounds__(kCurvBlock, PLIC_CURV_MINBLOCKS)
 curv_cells(const float *__restrict__ phi, float *__restrict__ kappa, int nx, int ny,
            const int *__restrict__ list, int capacity) {
     // launched with programmatic stream serialization: the blocks may become resident while
-    // curv_mark4 drains; nothing of its output is read before this wait
+    // curv_mark drains; nothing of its output is read before this wait
     asm volatile("griddepcontrol.wait;" ::: "memory");
     const int found = list[0];
     const int count = found < capacity ? found : capacity;
     const int64_t sy = nx, sz = (int64_t)nx * ny;
-    for (int j = blockIdx.x * kCurvBlock + threadIdx.x; j < count; j += gridDim.x * kCurvBlock) {
-        const int64_t c = list[1 + j];
-        float p[27];
-#pragma unroll
-        for (int i = 0; i < 27; ++i)
-            p[i] = __ldg(phi + c + (i % 3 - 1) + ((i / 3) % 3 - 1) * sy + (i / 9 - 1) * sz);
-        kappa[c] = curvature_point(p);
+    const int sub = threadIdx.x % kPointLanes;
+    const int per = kCurvBlock / kPointLanes;
+    for (int j0 = blockIdx.x * per; j0 < count; j0 += gridDim.x * per) {     // uniform per block
+        const int j = j0 + threadIdx.x / kPointLanes;
+        const bool live = j < count;
+        const int64_t c = list[1 + (live ? j : count - 1)];
+        const float k = curvature_point<kPointLanes>(phi, c, sy, sz, sub);
+        if (live && sub == 0) kappa[c] = k;
     }
 }
 

@@ -783,8 +783,8 @@ int plic_curvature(const float *phi, float *kappa, int nx, int ny, int nz, int32
         plic::curv_mark<<<(int)(need < full ? need : full), 256, 0, stream>>>(phi, kappa, nx, ny, nz,
                                                                              work, capacity);
     }
-    need = ((int64_t)capacity + plic::kCurvBlock - 1) / plic::kCurvBlock;
-    full = (int64_t)info->sms * 32;
+    need = ((int64_t)capacity * plic::kPointLanes + plic::kCurvBlock - 1) / plic::kCurvBlock;
+    full = (int64_t)info->sms * 16;
     {   // programmatic dependent launch: hides the launch latency behind the tail of the marking pass
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3((unsigned)(need < full ? need : full));

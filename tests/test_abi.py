@@ -90,13 +90,14 @@ def test_argument_validation_needs_no_device(plic):
     assert lib.plic_solve(p, p, p, p, p, 4, 0x204, None) == -3
     assert lib.plic_solve(p, p, p, p, p, 4, 0x104, None) == -3               # kawano has no fast form
     assert lib.plic_solve_host(p, p, p, p, p, 4, -1) == -3
-    # plic_roundtrip_error: sizes, method (blank allowed here, not in plic_solve), null
+    # plic_roundtrip_error: sizes, method, null
     assert lib.plic_roundtrip_error(None, None, None, None, 0, 256, 0, None) == 0
     assert lib.plic_roundtrip_error(p, p, p, p, 4, 1, 0, None) == -2
     assert lib.plic_roundtrip_error(p, p, p, p, -4, 256, 0, None) == -2
     assert lib.plic_roundtrip_error(p, p, p, p, 4, 256, 9, None) == -3
     assert lib.plic_roundtrip_error(p, p, None, p, 4, 256, 0x40, None) == -1
-    assert lib.plic_solve(p, p, p, p, p, 4, 0x40, None) == -3
+    assert lib.plic_solve(p, p, p, p, p, 4, 0x140, None) == -3              # blank has no fast form
+    assert lib.plic_solve(p, None, p, p, p, 4, 0x40, None) == -1            # blank is a plic_solve method (stream ceiling)
     # plane-sphere entry points
     assert lib.plic_sphere_solve(None, None, 0, 0, None) == 0
     assert lib.plic_sphere_solve(p, p, -1, 0, None) == -2
