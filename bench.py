@@ -458,22 +458,28 @@ def run_ours(args):
         methods[name] = timed_map(name, fn, 8)
 
     # ---- fp16-storage and fp64 variants of the solve ----------------------------
+    # the same cells: the fp32 workload rounded to binary16 (10 B per cell) resp. promoted to fp64 (40 B)
     storage = None
-    if hasattr(plic, "plic_solve_h") and not args.no_storage:
+    if not args.no_storage:
         storage = {}
         hV, hx, hy, hz = [t.half() for t in (dV, dx, dy, dz)]
         hout = torch.empty_like(hV)
-        for m in ("analytic", "sz", "newton", "nested"):
-            storage["%s-fast/f16" % m] = timed_map(
-                "%s-fast/f16" % m, lambda: plic.plic_solve_h(hV, hx, hy, hz, out=hout, method=m), 10)
-        storage["analytic-fast/f16in-f32out"] = timed_map(
-            "analytic-fast/f16in-f32out", lambda: plic.plic_solve_h(hV, hx, hy, hz, out=out, method="analytic"), 12)
+        storage["blank/f16"] = timed_map("blank/f16", lambda: plic.plic_solve_h(hV, hx, hy, hz, out=hout, method="blank"), 10)
+        for m, f in VARIANTS:
+            name = plic.plic_method_name(plic.method_id(m, f)) + "/f16"
+            storage[name] = timed_map(name, lambda: plic.plic_solve_h(hV, hx, hy, hz, out=hout, method=m, fast=f), 10)
+        storage["analytic-fast/f16+f32out"] = timed_map(
+            "analytic-fast/f16+f32out",
+            lambda: plic.plic_solve_h(hV, hx, hy, hz, out=hout, out_f32=out, method="analytic", fast=True), 14)
+        storage["plic_volume/f16"] = timed_map("plic_volume/f16", lambda: plic.plic_volume_h(hout, hx, hy, hz, out=hV), 10)
         del hV, hx, hy, hz, hout
         fV, fx, fy, fz = [t.double() for t in (dV, dx, dy, dz)]
         fout = torch.empty_like(fV)
-        for m in ("analytic", "sz"):
+        for m in ("analytic", "sz", "newton", "nested"):
             storage["%s/f64" % m] = timed_map("%s/f64" % m, lambda: plic.plic_solve_f64(fV, fx, fy, fz, out=fout, method=m), 40)
         del fV, fx, fy, fz, fout
+        for k, e in storage.items():
+            e["dtype"] = "f64" if k.endswith("/f64") else "f16 storage, f32 arithmetic"
     total_launches = plic.plic_launch_count() - launches_before
 
     solve_names = [plic.plic_method_name(plic.method_id(m, f)) for m, f in VARIANTS]

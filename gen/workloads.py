@@ -54,11 +54,11 @@ def _chunk_spans(start: int, count: int):
         c += 1
 
 
-def _run_chunks(fn, start, count, workers):
-    V0 = np.empty(count, dtype=np.float32)
-    nx = np.empty(count, dtype=np.float32)
-    ny = np.empty(count, dtype=np.float32)
-    nz = np.empty(count, dtype=np.float32)
+def _run_chunks(fn, start, count, workers, dtype=np.float32):
+    V0 = np.empty(count, dtype=dtype)
+    nx = np.empty(count, dtype=dtype)
+    ny = np.empty(count, dtype=dtype)
+    nz = np.empty(count, dtype=dtype)
 
     def work(span):
         c, lo, hi, o = span
@@ -81,22 +81,24 @@ def _run_chunks(fn, start, count, workers):
     return V0, nx, ny, nz
 
 
-def random_sphere(N: int, seed: int, start: int = 0, workers: int | None = None):
+def random_sphere(N: int, seed: int, start: int = 0, workers: int | None = None, dtype=np.float32):
     """Config 1 (random part) and config 2: normals uniform on the unit sphere
-    (normalised i.i.d. N(0,1) 3-vectors), V0 ~ U[0,1).  Returns fp32 (V0, nx, ny, nz)
-    for the cells [start, start+N) of the stream keyed by `seed`."""
+    (normalised i.i.d. N(0,1) 3-vectors), V0 ~ U[0,1).  Returns (V0, nx, ny, nz)
+    for the cells [start, start+N) of the stream keyed by `seed`, in `dtype`: fp32 (the
+    paper's type), or the same fp64 draws rounded once to fp16 or kept in fp64 (the
+    storage variants plic_solve_h / plic_solve_f64)."""
     def chunk(c):
         rng = _rng(seed, _STREAM_SPHERE, c)
         g = rng.standard_normal((CHUNK, 3))
         u = rng.random(CHUNK)
-        return u.astype(np.float32), _unit_rows(g).astype(np.float32)
-    return _run_chunks(chunk, start, N, workers)
+        return u.astype(dtype), _unit_rows(g).astype(dtype)
+    return _run_chunks(chunk, start, N, workers, dtype)
 
 
 EDGE_V0 = np.array([0.0, 0.5, 1.0, 1e-7, 1.0 - 1e-7], dtype=np.float32)
 
 
-def edge_cells(count: int = 4096, seed: int = 0):
+def edge_cells(count: int = 4096, seed: int = 0, dtype=np.float32):
     """Config 1 edge part: normals with one or two components exactly 0 (random
     signs, survivors random and renormalised; a single survivor is exactly +-1),
     V0 cycling through {0, 0.5, 1, 1e-7, 1-1e-7} (the last rounds to 0.99999988f).
@@ -111,15 +113,16 @@ def edge_cells(count: int = 4096, seed: int = 0):
     keep[two] = False
     keep[two, k[two]] = True                      # two zeros: only component k survives
     g = np.where(keep, g, 0.0)
-    n = _unit_rows(g).astype(np.float32)
-    V0 = EDGE_V0[j % 5].copy()
+    n = _unit_rows(g).astype(dtype)
+    # the five volumes in `dtype`: 1e-7 is subnormal in fp16 (1.19e-7) and 1 - 1e-7 rounds to 1 there
+    V0 = np.array([0.0, 0.5, 1.0, 1e-7, 1.0 - 1e-7], dtype=np.float64).astype(dtype)[j % 5].copy()
     return V0, n[:, 0].copy(), n[:, 1].copy(), n[:, 2].copy()
 
 
-def config1(seed: int = 0, n_random: int = 1 << 20, n_edge: int = 4096):
+def config1(seed: int = 0, n_random: int = 1 << 20, n_edge: int = 4096, dtype=np.float32):
     """BASELINE.json configs[0]: n_random random cells followed by n_edge edge cells."""
-    a = random_sphere(n_random, seed)
-    b = edge_cells(n_edge, seed)
+    a = random_sphere(n_random, seed, dtype=dtype)
+    b = edge_cells(n_edge, seed, dtype=dtype)
     return tuple(np.concatenate([x, y]) for x, y in zip(a, b))
 
 

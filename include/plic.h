@@ -62,7 +62,7 @@ typedef struct CUstream_st *cudaStream_t;
                                    negative lattice extents or more than 2^31-1 lattice cells */
 #define PLIC_ERR_METHOD      -3 /* unknown method id */
 #define PLIC_ERR_LAUNCH      -4 /* the CUDA runtime reported an error (launch, copy, alloc) */
-#define PLIC_ERR_ALIGN       -5 /* a pointer is not 4-byte aligned */
+#define PLIC_ERR_ALIGN       -5 /* a pointer is not aligned to its element size (4 bytes for fp32) */
 
 /*
  * plic_solve -- d0[i] = d0(V0[i], n[i]) for i in [0, N)            (eq. (1))
@@ -103,6 +103,52 @@ int plic_solve(const float *V0, const float *nx, const float *ny, const float *n
  */
 int plic_volume(const float *d0, const float *nx, const float *ny, const float *nz,
                 float *V0, int64_t N, cudaStream_t stream);
+
+/*
+ * plic_solve_h / plic_volume_h -- plic_solve / plic_volume on IEEE binary16 ("half") STORAGE with
+ * fp32 ARITHMETIC (the paper itself fixes fp32 storage and arithmetic,
+ * PAPER.md:254-256).  10 B of HBM traffic per cell instead of 20, so the HBM roofline doubles and the
+ * kernels are bound by instruction issue instead.
+ *
+ *   V0, nx, ny, nz  DEVICE pointers to N binary16 values each (bit patterns in uint16_t), read only.
+ *   d0              DEVICE pointer, N binary16 values, written: the fp32 result of the same arithmetic
+ *                   as plic_solve (each input converted exactly), rounded to nearest even.  May be the
+ *                   same pointer as V0.
+ *   d0_f32          optional DEVICE pointer (NULL to skip), N fp32 values, written: the result BEFORE
+ *                   it is rounded to binary16 (+4 B per cell).  d0 is bitwise the rounding of d0_f32.
+ *                   This is what the parity tests hold to the 2e-5 bound; d0 itself is within that
+ *                   bound plus half a binary16 ulp (2.4e-4 at |d0| in [1/2, 1)).
+ *   method          as plic_solve: PLIC_METHOD_* [| PLIC_FAST], PLIC_METHOD_KAWANO, PLIC_METHOD_BLANK.
+ *
+ * Pointers need only be 2-byte aligned (d0_f32: 4-byte); when the five binary16 pointers share one
+ * alignment modulo 16 (and d0_f32 + the head count is 16-byte aligned) the body runs on 128-bit or
+ * 64-bit accesses, 8 or 4 cells per thread, otherwise on a scalar kernel with bitwise equal results.
+ * Input domain, errors, ownership and stream semantics as plic_solve (PLIC_ERR_ALIGN for an odd
+ * address).  The normal as stored is no longer of unit length (binary16 rounding, <= 5e-4 relative);
+ * every method is homogeneous in n, so the result is the exact offset for the stored normal.
+ */
+int plic_solve_h(const uint16_t *V0, const uint16_t *nx, const uint16_t *ny, const uint16_t *nz,
+                 uint16_t *d0, float *d0_f32, int64_t N, int method, cudaStream_t stream);
+int plic_volume_h(const uint16_t *d0, const uint16_t *nx, const uint16_t *ny, const uint16_t *nz,
+                  uint16_t *V0, float *V0_f32, int64_t N, cudaStream_t stream);
+
+/*
+ * plic_solve_f64 -- plic_solve in fp64 storage AND arithmetic: 40 B of HBM
+ * traffic per cell; IEEE division and square root, CUDA libm cbrt / asin / sin / acos / cos in double
+ * precision; the like-for-like GPU counterpart of the fp64 bisection oracle.
+ *
+ *   V0, nx, ny, nz, d0   DEVICE pointers, fp64, N elements each (d0 may be the same pointer as V0).
+ *   method               PLIC_METHOD_ANALYTIC, _SZ, _NEWTON or _NESTED.  There is no PLIC_FAST form
+ *                        (the SFU approximations are fp32) and no Kawano / blank method:
+ *                        PLIC_ERR_METHOD.
+ *
+ * Same formulation as the precise fp32 kernels (a-priori case selection, depressed cubics, heavy
+ * cases compacted per tile); Newton-Raphson takes 7 steps for cases (3)/(4) and 6 for case (1), nested
+ * intervals halves until the fp64 midpoint stops moving.  Pointers must be 8-byte aligned; a common
+ * alignment modulo 16 selects the 128-bit body.  Errors, ownership and stream semantics as plic_solve.
+ */
+int plic_solve_f64(const double *V0, const double *nx, const double *ny, const double *nz, double *d0,
+                   int64_t N, int method, cudaStream_t stream);
 
 /*
  * plic_roundtrip_error -- the paper's accuracy and timing benchmark (sect. 2.6):
@@ -205,7 +251,8 @@ const char *plic_method_name(int method);
 const char *plic_error_string(int code);
 
 /* ABI version: 100*major + minor (1.04: + plic_roundtrip_error, plic_sphere_*, plic_curvature,
- * PLIC_METHOD_KAWANO). */
+ * PLIC_METHOD_KAWANO; 1.05: + plic_solve_h, plic_volume_h, plic_solve_f64, PLIC_METHOD_BLANK in
+ * plic_solve). */
 int plic_version(void);
 
 /*
@@ -216,7 +263,8 @@ int plic_version(void);
  * stores in *warp_instructions (HOST pointer) how many warp-instructions of that kind the launch
  * executes; the caller times the launch (CUDA events) and divides.
  *   pipe  0 scalar FFMA, 1 packed FFMA2, 2 MUFU (rsqrt), 3 FMNMX (ALU pipe), 4 LOP3 (ALU pipe),
- *         5 the halving step of nested-fast (2 FFMA2 + 2 LOP3 + FADD2 per pair)
+ *         5 the halving step of nested-fast (2 FFMA2 + 2 LOP3 + FADD2 per pair), 6-16 mixes of these
+ *         (names in the Python binding's PROBES), 17 fp64 FMA
  *   trips loop trips per thread, >= 0 (64 instructions per chain set and trip; 320 for pipe 5)
  *   sink  DEVICE pointer to >= 256 floats (never written in practice; keeps the chains alive)
  * Returns PLIC_OK or PLIC_ERR_METHOD (unknown pipe) / _SIZE / _NULL / _LAUNCH.

@@ -10,6 +10,8 @@ shared library is missing it is built with nvcc, and if that fails the import ra
     plic_solve(V0, nx, ny, nz, out=None, method="analytic", fast=False, stream=None) -> d0
     plic_volume(d0, nx, ny, nz, out=None, stream=None) -> V0
     plic_solve_host / plic_volume_host      same maps for host arrays (numpy or CPU tensors)
+    plic_solve_h / plic_volume_h            the same maps on float16 tensors (fp32 arithmetic, 10 B/cell)
+    plic_solve_f64                          plic_solve on float64 tensors in fp64 arithmetic (40 B/cell)
     plic_roundtrip_error(nx, ny, nz, L, out=None, method="analytic", fast=False) -> E
                                             the paper's benchmark loop, eq. (31)-(33)
     plic_sphere_solve(V0, out=None, fast=False) -> d0, plic_sphere_volume(d0, out=None) -> V0
@@ -25,6 +27,7 @@ import os
 from . import build as _build
 
 __all__ = ["METHODS", "FAST", "BLANK", "KAWANO", "method_id", "plic_solve", "plic_volume",
+           "plic_solve_h", "plic_volume_h", "plic_solve_f64",
            "plic_roundtrip_error", "plic_sphere_solve", "plic_sphere_volume", "plic_curvature",
            "plic_solve_host",
            "plic_volume_host", "plic_host_release", "plic_method_name", "plic_error_string",
@@ -54,6 +57,12 @@ def _load() -> ctypes.CDLL:
     lib_.plic_solve.restype = ctypes.c_int
     lib_.plic_volume.argtypes = [fp, fp, fp, fp, fp, i64, ctypes.c_void_p]
     lib_.plic_volume.restype = ctypes.c_int
+    lib_.plic_solve_h.argtypes = [fp, fp, fp, fp, fp, fp, i64, ctypes.c_int, ctypes.c_void_p]
+    lib_.plic_solve_h.restype = ctypes.c_int
+    lib_.plic_volume_h.argtypes = [fp, fp, fp, fp, fp, fp, i64, ctypes.c_void_p]
+    lib_.plic_volume_h.restype = ctypes.c_int
+    lib_.plic_solve_f64.argtypes = [fp, fp, fp, fp, fp, i64, ctypes.c_int, ctypes.c_void_p]
+    lib_.plic_solve_f64.restype = ctypes.c_int
     lib_.plic_roundtrip_error.argtypes = [fp, fp, fp, fp, i64, ctypes.c_int, ctypes.c_int,
                                           ctypes.c_void_p]
     lib_.plic_roundtrip_error.restype = ctypes.c_int
@@ -137,7 +146,7 @@ def plic_launch_config(method, N: int, fast: bool = False):
 
 PROBES = {"ffma": 0, "ffma2": 1, "mufu": 2, "fmnmx": 3, "lop3": 4, "nested_step": 5, "ffma+lop3": 6,
           "ffma2+lop3": 7, "mufu+4ffma": 8, "ffma+fmnmx": 9, "fsetp+fsel": 10, "nested_step_scalar": 11,
-          "nested_step_hybrid": 12, "fadd": 13, "fmul": 14, "fadd2": 15, "2ffma+lop3+fadd": 16}
+          "nested_step_hybrid": 12, "fadd": 13, "fmul": 14, "fadd2": 15, "2ffma+lop3+fadd": 16, "dfma": 17}
 
 
 def plic_pipe_probe(pipe, trips: int, sink, stream=None) -> int:
@@ -159,20 +168,32 @@ def plic_host_release() -> None:
 # ------------------------------------------------------------------------------------------
 # device-pointer API (torch CUDA tensors)
 # ------------------------------------------------------------------------------------------
-def _device_args(first, nx, ny, nz, out):
+def _device_args(first, nx, ny, nz, out, dtype=None):
     import torch
+    dtype = torch.float32 if dtype is None else dtype
     N = first.numel()
     for t in (first, nx, ny, nz):
-        if not (t.is_cuda and t.dtype == torch.float32 and t.dim() == 1 and t.is_contiguous()
+        if not (t.is_cuda and t.dtype == dtype and t.dim() == 1 and t.is_contiguous()
                 and t.numel() == N and t.device == first.device):
-            raise ValueError("inputs must be contiguous 1-D float32 CUDA tensors of one length "
-                             "on one device")
+            raise ValueError("inputs must be contiguous 1-D %s CUDA tensors of one length "
+                             "on one device" % (dtype,))
     if out is None:
         out = torch.empty_like(first)
-    elif not (out.is_cuda and out.dtype == torch.float32 and out.is_contiguous()
+    elif not (out.is_cuda and out.dtype == dtype and out.is_contiguous()
               and out.numel() == N and out.device == first.device):
-        raise ValueError("out must be a contiguous float32 CUDA tensor of the inputs' length")
+        raise ValueError("out must be a contiguous %s CUDA tensor of the inputs' length" % (dtype,))
     return N, out
+
+
+def _aux_ptr(aux, N, device):
+    """Optional float32 side output of the binary16 maps: data pointer or None."""
+    import torch
+    if aux is None:
+        return None
+    if not (aux.is_cuda and aux.dtype == torch.float32 and aux.is_contiguous() and aux.numel() == N
+            and aux.device == device):
+        raise ValueError("out_f32 must be a contiguous float32 CUDA tensor of the inputs' length")
+    return aux.data_ptr()
 
 
 def _stream_handle(stream, device):
@@ -204,6 +225,44 @@ def plic_volume(d0, nx, ny, nz, out=None, stream=None):
                              out.data_ptr(), N, _stream_handle(stream, d0.device))
     if rc != 0:
         raise PlicError(rc, "plic_volume")
+    return out
+
+
+def plic_solve_h(V0, nx, ny, nz, out=None, out_f32=None, method="analytic", fast: bool = False, stream=None):
+    """plic_solve on float16 tensors (binary16 storage, fp32 arithmetic); `out_f32`, if given, also
+    receives the float32 result before it is rounded to float16.  Returns `out` (float16)."""
+    import torch
+    N, out = _device_args(V0, nx, ny, nz, out, torch.float16)
+    with torch.cuda.device(V0.device):
+        rc = lib.plic_solve_h(V0.data_ptr(), nx.data_ptr(), ny.data_ptr(), nz.data_ptr(), out.data_ptr(),
+                              _aux_ptr(out_f32, N, V0.device), N, method_id(method, fast),
+                              _stream_handle(stream, V0.device))
+    if rc != 0:
+        raise PlicError(rc, "plic_solve_h")
+    return out
+
+
+def plic_volume_h(d0, nx, ny, nz, out=None, out_f32=None, stream=None):
+    """plic_volume on float16 tensors (binary16 storage, fp32 arithmetic).  Returns `out` (float16)."""
+    import torch
+    N, out = _device_args(d0, nx, ny, nz, out, torch.float16)
+    with torch.cuda.device(d0.device):
+        rc = lib.plic_volume_h(d0.data_ptr(), nx.data_ptr(), ny.data_ptr(), nz.data_ptr(), out.data_ptr(),
+                               _aux_ptr(out_f32, N, d0.device), N, _stream_handle(stream, d0.device))
+    if rc != 0:
+        raise PlicError(rc, "plic_volume_h")
+    return out
+
+
+def plic_solve_f64(V0, nx, ny, nz, out=None, method="analytic", stream=None):
+    """plic_solve on float64 tensors in fp64 arithmetic (precise methods only).  Returns `out`."""
+    import torch
+    N, out = _device_args(V0, nx, ny, nz, out, torch.float64)
+    with torch.cuda.device(V0.device):
+        rc = lib.plic_solve_f64(V0.data_ptr(), nx.data_ptr(), ny.data_ptr(), nz.data_ptr(), out.data_ptr(),
+                                N, method_id(method, False), _stream_handle(stream, V0.device))
+    if rc != 0:
+        raise PlicError(rc, "plic_solve_f64")
     return out
 
 

@@ -28,7 +28,7 @@
 #include "plic_curvature.cuh"
 #include "plic_probe.cuh"
 
-#define PLIC_VERSION 104
+#define PLIC_VERSION 105
 
 namespace plic {
 
@@ -715,6 +715,8 @@ static int host_map(int k, const float *s, const float *nx, const float *ny, con
 
 }  // namespace plic
 
+#include "plic_storage.cuh"       // binary16-storage and fp64 variants (uses the kernels and helpers above)
+
 // ---------------------------------------------------------------------------------------
 // C ABI
 // ---------------------------------------------------------------------------------------
@@ -730,6 +732,25 @@ int plic_solve(const float *V0, const float *nx, const float *ny, const float *n
 int plic_volume(const float *d0, const float *nx, const float *ny, const float *nz, float *V0,
                 int64_t N, cudaStream_t stream) {
     return plic::launch_map(plic::kVolumeKernel, d0, nx, ny, nz, V0, N, stream);
+}
+
+int plic_solve_h(const uint16_t *V0, const uint16_t *nx, const uint16_t *ny, const uint16_t *nz,
+                 uint16_t *d0, float *d0_f32, int64_t N, int method, cudaStream_t stream) {
+    const int k = plic::kernel_index(method);
+    if (k < 0) return PLIC_ERR_METHOD;
+    return plic::launch_map_io(plic::io_kernel_h(k), 2, V0, nx, ny, nz, d0, d0_f32, N, stream);
+}
+
+int plic_volume_h(const uint16_t *d0, const uint16_t *nx, const uint16_t *ny, const uint16_t *nz,
+                  uint16_t *V0, float *V0_f32, int64_t N, cudaStream_t stream) {
+    return plic::launch_map_io(plic::io_kernel_h(plic::kVolumeKernel), 2, d0, nx, ny, nz, V0, V0_f32, N, stream);
+}
+
+int plic_solve_f64(const double *V0, const double *nx, const double *ny, const double *nz, double *d0,
+                   int64_t N, int method, cudaStream_t stream) {
+    const int k = plic::kernel_index(method);
+    if (k < 0) return PLIC_ERR_METHOD;
+    return plic::launch_map_io(plic::io_kernel_d(k), 8, V0, nx, ny, nz, d0, nullptr, N, stream);
 }
 
 int plic_roundtrip_error(const float *nx, const float *ny, const float *nz, float *E, int64_t N,
@@ -845,7 +866,7 @@ const char *plic_error_string(int code) {
         case PLIC_ERR_SIZE: return "size argument out of range";
         case PLIC_ERR_METHOD: return "unknown method id";
         case PLIC_ERR_LAUNCH: return "CUDA runtime error";
-        case PLIC_ERR_ALIGN: return "pointer not 4-byte aligned";
+        case PLIC_ERR_ALIGN: return "pointer not aligned to its element size";
         default: return "unknown error code";
     }
 }
@@ -880,6 +901,10 @@ int plic_pipe_probe(int pipe, int trips, float *sink, int64_t *warp_instructions
         PLIC_PROBE_CASE(PROBE_FMUL)
         PLIC_PROBE_CASE(PROBE_FADD2)
         PLIC_PROBE_CASE(PROBE_3FP_LOP3)
+        case plic::PROBE_DFMA:
+            plic::pipe_probe_dfma<<<grid, plic::kBlock, 0, stream>>>(sink, trips);
+            per_trip = (int64_t)plic::kProbeChains * plic::kProbeUnroll;
+            break;
         case plic::PROBE_NESTED_SCALAR:
             plic::pipe_probe_nested_alt<0><<<grid, plic::kBlock, 0, stream>>>(sink, trips);
             per_trip = 4 * 16 * 8;                               // 4 pairs x 16 halvings x 8 instructions

@@ -13,6 +13,7 @@
 //   PROBE_FMNMX   fp32 min/max                   (ALU pipe: min/max, compare, select, logic)
 //   PROBE_LOP3    32-bit logic op                (ALU pipe; the sign transfer of nested-fast)
 //   PROBE_NESTED  the nested-fast halving step   (2 FFMA2 + 2 LOP3 + 1 FADD2 per pair)
+//   PROBE_DFMA    fp64 FMA                       (the pipe that bounds plic_solve_f64)
 #pragma once
 #include "plic_packed.cuh"
 
@@ -21,7 +22,7 @@ namespace plic {
 enum : int { PROBE_FFMA = 0, PROBE_FFMA2 = 1, PROBE_MUFU = 2, PROBE_FMNMX = 3, PROBE_LOP3 = 4, PROBE_NESTED = 5,
              PROBE_FFMA_LOP3 = 6, PROBE_FFMA2_LOP3 = 7, PROBE_MUFU_FFMA4 = 8, PROBE_FFMA_FMNMX = 9, PROBE_FSEL = 10,
              PROBE_NESTED_SCALAR = 11, PROBE_NESTED_HYBRID = 12, PROBE_FADD = 13, PROBE_FMUL = 14, PROBE_FADD2 = 15,
-             PROBE_3FP_LOP3 = 16, PROBE_COUNT = 17 };
+             PROBE_3FP_LOP3 = 16, PROBE_DFMA = 17, PROBE_COUNT = 18 };
 constexpr int kProbeChains = 8;        // independent chains per thread
 constexpr int kProbeUnroll = 8;        // instructions per chain per loop trip
 constexpr int kProbeBlocksPerSm = 8;   // x 256 threads = 16 warps per sub-partition
@@ -182,6 +183,24 @@ pipe_probe(float *sink, int trips) {
         else acc += a[j];
     }
     if (acc == 123456.789f) sink[threadIdx.x] = acc;      // never true: keeps the chains alive
+}
+
+// fp64 FMA in 8 independent chains per thread (kProbeChains x kProbeUnroll instructions per trip)
+__global__ void __launch_bounds__(256)
+pipe_probe_dfma(float *sink, int trips) {
+    double a[kProbeChains];
+    const double seed = 1.0 + (double)threadIdx.x * (1.0 / 4096.0);
+    const double x = 0.999, y = seed * 1e-3;
+    for (int j = 0; j < kProbeChains; ++j) a[j] = seed + (double)j;
+    for (int t = 0; t < trips; ++t) {
+#pragma unroll
+        for (int u = 0; u < kProbeUnroll; ++u)
+#pragma unroll
+            for (int j = 0; j < kProbeChains; ++j) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(a[j]) : "d"(x), "d"(y));
+    }
+    double acc = 0.0;
+    for (int j = 0; j < kProbeChains; ++j) acc += a[j];
+    if (acc == 123456.789) sink[threadIdx.x] = (float)acc;
 }
 
 // the halving step of PairSolver<NESTED> on 4 independent pairs per thread

@@ -47,7 +47,7 @@ def test_header_compiles_as_plain_c(tmp_path):
 
 
 def test_version_and_names(plic):
-    assert plic.plic_version() == 104
+    assert plic.plic_version() == 105
     assert [plic.plic_method_name(i) for i in range(4)] == ["analytic", "sz", "newton", "nested"]
     assert plic.plic_method_name(2 | plic.FAST) == "newton-fast"
     assert plic.plic_method_name(4) == "kawano" and plic.plic_method_name(4 | plic.FAST) is None
@@ -90,6 +90,22 @@ def test_argument_validation_needs_no_device(plic):
     assert lib.plic_solve(p, p, p, p, p, 4, 0x204, None) == -3
     assert lib.plic_solve(p, p, p, p, p, 4, 0x104, None) == -3               # kawano has no fast form
     assert lib.plic_solve_host(p, p, p, p, p, 4, -1) == -3
+    # storage variants: same validation order; fp64 has the four precise methods only
+    assert lib.plic_solve_h(None, None, None, None, None, None, 0, 0, None) == 0
+    assert lib.plic_solve_h(p, p, p, p, p, None, -1, 0, None) == -2
+    assert lib.plic_solve_h(p, p, None, p, p, None, 4, 0x100, None) == -1
+    assert lib.plic_solve_h(p, p, p, p, p, None, 4, 0x204, None) == -3
+    assert lib.plic_solve_h(ctypes.c_void_p(p.value + 1), p, p, p, p, None, 4, 0, None) == -5
+    assert lib.plic_solve_h(p, p, p, p, p, ctypes.c_void_p(p.value + 2), 4, 0, None) == -5
+    assert lib.plic_volume_h(None, None, None, None, None, None, 0, None) == 0
+    assert lib.plic_volume_h(p, p, p, None, p, None, 4, None) == -1
+    assert lib.plic_solve_f64(None, None, None, None, None, 0, 0, None) == 0
+    assert lib.plic_solve_f64(p, p, p, p, p, -1, 0, None) == -2
+    assert lib.plic_solve_f64(p, p, p, p, None, 2, 3, None) == -1
+    assert lib.plic_solve_f64(p, p, p, p, p, 2, 0x100, None) == -3             # no fast form in fp64
+    assert lib.plic_solve_f64(p, p, p, p, p, 2, 4, None) == -3                 # no kawano
+    assert lib.plic_solve_f64(p, p, p, p, p, 2, 0x40, None) == -3              # no blank
+    assert lib.plic_solve_f64(ctypes.c_void_p(p.value + 4), p, p, p, p, 2, 0, None) == -5
     # plic_roundtrip_error: sizes, method, null
     assert lib.plic_roundtrip_error(None, None, None, None, 0, 256, 0, None) == 0
     assert lib.plic_roundtrip_error(p, p, p, p, 4, 1, 0, None) == -2
