@@ -19,9 +19,10 @@ variant after 0.5 s of idle, at full clocks -- the regime MEASURED_PEAKS.json's 
 was taken in.
 
 Per method: `hbm_frac` against the measured copy bandwidth and `hbm_frac_nominal`
-against 8 TB/s; `issue_frac` = warp-instructions per cell (ncu's executed count, from the committed
-table profiles/instruction_counts.txt) x cells/s / (SMs x 4 schedulers x the SM clock sampled in
-that method's timed window); `bound` names the larger of the two fractions.  "stream_ceiling" is the
+against 8 TB/s; `issue_frac` = issue slots per cell x cells/s / (SMs x 4 sub-partitions x the SM
+clock sampled in that method's timed window), issue slots = warp-instructions (ncu's executed count)
++ packed fp32x2 warp-instructions (they hold the issue port for two clocks, see pipe_rates), both per
+cell from the committed table profiles/instruction_counts.txt; `bound` names the larger fraction.  "stream_ceiling" is the
 same 4-read/1-write stream with no arithmetic (plic_solve with the blank method, d0 = V0 - 1/2);
 "pipe_rates" are the instruction rates of the FMA, SFU and ALU pipes measured in this run
 (plic_pipe_probe), from which the "alu" peak of the compute-bound legs is derived.
@@ -377,15 +378,27 @@ def time_variants(plic, arrays, out, steps, warmup, stream, world, sampler, sms,
              "bytes_per_cell": BYTES_PER_CELL, "hbm_gbs_per_gpu": gbs, "hbm_frac": gbs / peak,
              "hbm_frac_nominal": gbs / NOMINAL_HBM_GBS, "sm_mhz": clk.get("sm_mhz")}
         e["roofline_frac"] = e["hbm_frac"]
-        row = counts.get(name)
-        if row is not None and clk.get("sm_mhz"):
-            wipc = float(row[0])
-            e["warp_inst_per_cell"] = wipc
-            e["lanes_per_inst"] = float(row[1])
-            e["issue_frac"] = wipc * N / (ms * 1e-3) / (sms * 4 * clk["sm_mhz"] * 1e6)
-            e["bound"] = "issue" if e["issue_frac"] > e["hbm_frac"] else "hbm"
+        issue_fields(e, counts.get(name), N, ms, sms, clk.get("sm_mhz"))
         res[name] = e
     return res
+
+
+def issue_fields(e, row, N, ms, sms, mhz):
+    """Issue roofline of one timed kernel from its row of profiles/instruction_counts.txt.  A packed
+    fp32x2 instruction (FFMA2/FMUL2/FADD2) holds the issue port of its SM sub-partition for two
+    clocks (pipe_rates: ffma2 alone 0.50 per clock, ffma2 + lop3 0.66 = 3 clocks per pair), every
+    other instruction for one, so issue slots per cell = warp-instructions + packed warp-instructions;
+    issue_frac = slots per cell x cells/s / (SMs x 4 sub-partitions x the SM clock sampled in this
+    kernel's timed window)."""
+    if row is None or not mhz:
+        return
+    wipc, packed = float(row[0]), float(row[2])
+    e["warp_inst_per_cell"] = wipc
+    e["lanes_per_inst"] = float(row[1])
+    e["packed_warp_inst_per_cell"] = packed
+    e["issue_slots_per_cell"] = wipc + packed
+    e["issue_frac"] = (wipc + packed) * N / (ms * 1e-3) / (sms * 4 * mhz * 1e6)
+    e["bound"] = "issue" if e["issue_frac"] > e["hbm_frac"] else "hbm"
 
 
 def run_ours(args):
@@ -438,11 +451,7 @@ def run_ours(args):
         e = {"value": N * world / (ms * 1e-3) / 1e9, "ms_per_step": ms, "launches": args.steps,
              "bytes_per_cell": bytes_per_cell, "hbm_gbs_per_gpu": gbs, "hbm_frac": gbs / peak,
              "hbm_frac_nominal": gbs / NOMINAL_HBM_GBS, "roofline_frac": gbs / peak, "sm_mhz": clk.get("sm_mhz")}
-        row = counts.get(name)
-        if row is not None and clk.get("sm_mhz"):
-            e["warp_inst_per_cell"] = float(row[0])
-            e["issue_frac"] = float(row[0]) * N / (ms * 1e-3) / (sms * 4 * clk["sm_mhz"] * 1e6)
-            e["bound"] = "issue" if e["issue_frac"] > e["hbm_frac"] else "hbm"
+        issue_fields(e, counts.get(name), N, ms, sms, clk.get("sm_mhz"))
         return e
 
     # the 4-read / 1-write stream with no arithmetic, in the same sustained regime
@@ -516,7 +525,10 @@ def run_ours(args):
             pipe_rates["probes"][name] = {"t_inst_per_s": n_inst / sec / 1e12, "sm_mhz": mhz, "ms": sec * 1e3,
                                           "per_smsp_clk": n_inst / sec / (sms * 4 * mhz * 1e6)}
         pipe_rates["reading"] = ("scalar FFMA/FADD/FMUL issue at ~1 per clock, packed fp32x2 and every ALU-pipe "
-                                 "instruction (min/max, compare, select, logic) at 1 per 2 clocks, MUFU at 1 per 8; "
+                                 "instruction (min/max, compare, select, logic) at 1 per 2 clocks, MUFU at 1 per 8; a "
+                                 "scalar FMA and an ALU instruction overlap (ffma+lop3 ~1 per clock) but a packed one and "
+                                 "an ALU instruction do not (ffma2+lop3 ~0.66 per clock = 3 clocks per pair): a packed "
+                                 "instruction holds the issue port for 2 clocks, which is the slot count issue_frac uses; "
                                  "nested_step* = one halving of nested-fast for a pair of cells in three encodings")
         del sink
 
@@ -547,18 +559,21 @@ def run_ours(args):
         row = counts.get("roundtrip:analytic-fast")
         mhz = sampler.summary([pwin["analytic-fast"]]).get("sm_mhz") or sampler.sm_max or 1965
         if row is not None:
-            wipe = float(row[0])
+            wipe, packed = float(row[0]), float(row[2])
             peak_wis = sms * 4 * mhz * 1e6 / 1e12
-            ach = wipe * PN * PL / (raw["analytic-fast"][0] * 1e-3) / 1e12
+            ach = (wipe + packed) * PN * PL / (raw["analytic-fast"][0] * 1e-3) / 1e12
             paper["roofline"] = {"bound": "alu", "kernel": "roundtrip_kernel<analytic, fast>", "achieved": ach,
-                                 "peak": peak_wis, "unit": "T warp-instructions/s", "frac": ach / peak_wis,
-                                 "warp_instructions_per_evaluation": wipe, "sm_mhz": mhz,
-                                 "counts_source": "profiles/instruction_counts.txt (ncu smsp__inst_executed.sum, commit %s)"
-                                                  % counts.get("@commit", ["?"])[0],
-                                 "peak_source": "%d SMs x 4 schedulers x 1 warp-instruction per clock at the sampled SM "
-                                                "clock; the scalar-FFMA probe of this run reaches %.2f of it, packed and "
-                                                "ALU-pipe instructions half of it (pipe_rates)" % (
-                                                    sms, pipe_rates["probes"]["ffma"]["per_smsp_clk"] if pipe_rates else float("nan"))}
+                                 "peak": peak_wis, "unit": "T issue slots/s", "frac": ach / peak_wis,
+                                 "warp_instructions_per_evaluation": wipe,
+                                 "packed_warp_instructions_per_evaluation": packed,
+                                 "issue_slots_per_evaluation": wipe + packed, "sm_mhz": mhz,
+                                 "counts_source": "profiles/instruction_counts.txt (ncu smsp__inst_executed.sum, packed "
+                                                  "instructions from the SASS, commit %s)" % counts.get("@commit", ["?"])[0],
+                                 "peak_source": "%d SMs x 4 sub-partitions x 1 issue slot per clock at the sampled SM clock; "
+                                                "a packed fp32x2 instruction takes two slots, any other one (pipe_rates: "
+                                                "scalar FFMA %.2f, FFMA2 %.2f, FFMA2+LOP3 %.2f instructions per clock)" % (
+                                                    sms, *([pipe_rates["probes"][k]["per_smsp_clk"] for k in
+                                                            ("ffma", "ffma2", "ffma2+lop3")] if pipe_rates else [float("nan")] * 3))}
         del pn, pE
 
     for k, v in methods.items():

@@ -173,6 +173,11 @@ constexpr int kTmaSmem = kTiles * 4 * kTileBytes + kTiles * 8;       // tiles + 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {
     return (uint32_t)__cvta_generic_to_shared(p);
 }
+__device__ __forceinline__ bool elect_one() {                        // one lane of the (converged) warp
+    unsigned pred;
+    asm volatile("{ .reg .pred p; elect.sync _|p, 0xffffffff; selp.u32 %0, 1, 0, p; }" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
 }
@@ -212,7 +217,11 @@ map_tma(const float4 *s, const float4 *__restrict__ nx, const float4 *__restrict
     const int tid = threadIdx.x;
     const int64_t ntiles = (n4 + kBlock - 1) / kBlock;
     const int64_t first = (int64_t)blockIdx.x * kTiles;
-    if (tid == 0) {
+    // one elected lane of warp 0 issues the copies; the warp index is broadcast so that the branch is
+    // provably warp-uniform (the bulk-copy instructions run on the uniform datapath: under a
+    // divergent branch ptxas wraps each of them in an election loop)
+    const bool issuer = __shfl_sync(0xffffffffu, tid >> 5, 0) == 0 && elect_one();
+    if (issuer) {
         for (int k = 0; k < kTiles; ++k) mbar_init(&full[k], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         grid_dependency_wait();                     // before the first read of global memory

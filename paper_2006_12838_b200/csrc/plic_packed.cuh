@@ -72,14 +72,15 @@ __device__ __forceinline__ F2 rcp2(F2 a) { return F2{mufu_rcp(a.x), mufu_rcp(a.y
 __device__ __forceinline__ F2 lg2_2(F2 a) { return F2{mufu_lg2(a.x), mufu_lg2(a.y)}; }
 __device__ __forceinline__ F2 ex2_2(F2 a) { return F2{mufu_ex2(a.x), mufu_ex2(a.y)}; }
 
-// -sin(asin(C)/3) for C in [0, 0.9], both halves.  g = sin(asin(C)/3) is the root in [0, 0.36]
-// of the triple-angle relation 3g - 4g^3 = C.  An odd minimax start value C*P3(C^2)
+// -sin(asin(C)/3) (TWICE: -2 sin(asin(C)/3)) for C in [0, 0.9], both halves.  g = sin(asin(C)/3) is the
+// root in [0, 0.36] of the triple-angle relation 3g - 4g^3 = C.  An odd minimax start value C*P3(C^2)
 // (|err| < 2.0e-4 on [0, 0.9]) is polished by one Newton step g <- (C - 8g^3)/(3 - 12g^2),
 // whose denominator stays >= 1.4; the result is within 1.3e-7 of the exact value.  This
 // replaces the asin + sin pair of the trigonometric cubic root (eq. (12)): the
 // argument range C <= 5/(4 sqrt 2) = 0.884 is a property of cases (3)/(4) ("trig
-// range").  The step's denominator is taken with the opposite sign, which negates the result
-// at no cost.  Coefficients: fit_coefficients.py.
+// range").  The step's denominator is taken with the opposite sign (and halved for TWICE), which
+// negates (doubles) the result at no cost.  Coefficients: fit_coefficients.py.
+template <bool TWICE>
 __device__ __forceinline__ F2 neg_sin_third_asin_fast2(F2 C) {
     const F2 C2 = mul2(C, C);
     F2 g = fma2(C2, f2(0.100619423f), f2(-0.0602495379f));
@@ -88,7 +89,7 @@ __device__ __forceinline__ F2 neg_sin_third_asin_fast2(F2 C) {
     g = mul2(g, C);
     const F2 g2 = mul2(g, g);
     const F2 num = fma2(mul2(g2, -8.0f), g, C);
-    const F2 den = fma2(g2, 12.0f, f2(-3.0f));
+    const F2 den = TWICE ? fma2(g2, 6.0f, f2(-1.5f)) : fma2(g2, 12.0f, f2(-3.0f));
     return mul2(num, rcp2(den));
 }
 
@@ -121,13 +122,20 @@ __device__ __forceinline__ PairIn pair_reduce(F2 V0, F2 nx, F2 ny, F2 nz) {
     return in;
 }
 
-// d0 = sign(V0 - 1/2) (S/2 - d), eq. (8).  d <= S/2 is enforced (also turns a NaN into S/2),
-// so r >= 0 and the sign is a bit operation: set when V0 <= 1/2.
-__device__ __forceinline__ F2 pair_restore(F2 V0, F2 hS, F2 d) {
-    const F2 r = sub2(hS, min2(d, hS));
+// d0 = sign(V0 - 1/2) (S/2 - d), eq. (8), from the residual r = S/2 - d >= 0: the sign is a bit
+// operation, set when V0 <= 1/2.
+__device__ __forceinline__ F2 pair_restore(F2 V0, F2 r) {
     const F2 t = fma2(V0, -1.0f, f2(0.5f));
     return F2{__uint_as_float(__float_as_uint(r.x) | (~__float_as_uint(t.x) & 0x80000000u)),
               __uint_as_float(__float_as_uint(r.y) | (~__float_as_uint(t.y) & 0x80000000u))};
+}
+
+// Last step of every method: the residual r = S/2 - d.  For cases (1)-(4) d <= S/2 is enforced
+// (which also turns a NaN into r = 0); in case (5), d5 = V n3 + n12/2 (eq. (25)) gives
+// r = S/2 - d5 = (n3 - W)/2 directly (W = 2 V n3 <= n3), one multiplication instead of forming d5.
+// h = (n3 - W)/2 is passed in because the iterative methods use it as well.
+__device__ __forceinline__ F2 pair_residual(const PairIn &in, F2 d, F2 W, F2 h) {
+    return sel2(le2(in.n12, W), h, sub2(in.hS, min2(d, in.hS)));                // (5) | (1)-(4)
 }
 
 // A-priori (3)-vs-(4) decision on a pair: case (4) iff n3 < n12 and F3(e) > 0 (is_case4()).
@@ -143,17 +151,41 @@ struct PairSolver;
 // method 0, PLIC_FAST: analytic inverse (eq. (25)/(26)) for two cells at once.  Every closed
 // form is evaluated and merged by select, (3)/(4) are chosen a priori and served by one
 // trigonometric evaluation, and there is no branch at all, so the two cells of a pair (and
-// the 32 lanes of a warp) share one instruction stream.  cbrt = ex2(lg2(x)/3).  With R = 8 q (case 3) or u (case 4) and rho = rsqrt(R):
-//   (3): d = n12 - sqrt(R) g(C),  C = (3/2) z rho           [2 sqrt(2q) = sqrt(8q)]
-//   (4): d = S/2 - sqrt(R) g(C),  C = 6 q (n3 - W) rho^3
-// Both roots are >= n2, which serves as the common floor (it also replaces a NaN from
-// R = 0, i.e. n1 n2 flushed to zero, where the bracket [n2, n12] is narrower than fp32).
+// the 32 lanes of a warp) share one instruction stream.  cbrt = ex2(lg2(x)/3).
+// With R = 2 q (case 3) or u/4 (case 4) and rho = rsqrt(R), both cases read
+//   d = base - 2 R rho g(C),   C = (3/4) rho {z | q (n3 - W) rho^2},   base = {n12 | S/2}
+// [(3): 2 sqrt(2q) = 2 R rho, C3 = 3 z / (4 sqrt(2q));  (4): sqrt(u) = 2 R rho, C4 = 6 q (n3 - W) / u^(3/2)];
+// the factor 2 is folded into g's Newton step.  Both roots are >= n2, which serves as the common
+// floor (it also replaces a NaN from R = 0, i.e. n1 n2 flushed to zero, where the bracket
+// [n2, n12] is narrower than fp32).
 // ---------------------------------------------------------------------------------------
+// The part of cases (3)/(4) that the analytic and the SZ kernel share: R, rho, the argument C of
+// the trigonometric root, the case flag and h = (n3 - W)/2.
+struct Trig34 {
+    F2 R, rho, C, h;
+    B2 c4;
+};
+__device__ __forceinline__ Trig34 trig34(const PairIn &in, F2 W) {
+    Trig34 t;
+    const F2 q = mul2(in.n1, in.n2);
+    const F2 e = sub2(in.n3, in.n12);
+    const F2 z = sub2(in.n12, W);
+    const F2 ee = mul2(e, e);
+    const F2 n3mW = sub2(in.n3, W);
+    t.h = mul2(n3mW, 0.5f);
+    t.c4 = is_case4_2(q, e, ee, z);
+    t.R = sel2(t.c4, fma2(ee, -0.25f, q), add2(q, q));                          // u/4 | 2 q
+    t.rho = rsqrt2(t.R);
+    const F2 K4 = mul2(mul2(q, n3mW), mul2(t.rho, t.rho));
+    t.C = mul2(sel2(t.c4, K4, z), mul2(t.rho, 0.75f));
+    return t;
+}
+
 template <>
 struct PairSolver<ANALYTIC> {
-    static __device__ __forceinline__ F2 reduced_offset(const PairIn &in) {
-        const F2 n1 = in.n1, n2 = in.n2, n3 = in.n3, n12 = in.n12;
-        const F2 W = mul2(in.V2, n3);                                           // 2 V n3
+    static __device__ __forceinline__ F2 residual(const PairIn &in) {
+        const F2 n1 = in.n1, n2 = in.n2, n12 = in.n12;
+        const F2 W = mul2(in.V2, in.n3);                                        // 2 V n3
         const F2 Wn2 = mul2(W, n2);                                             // x / 3, x = 6 V n2 n3
         const F2 s1 = mul2(n1, n1);
         const F2 t1 = fma2(s1, -1.0f / 3.0f, Wn2);                              // (x - n1^2) / 3
@@ -164,126 +196,122 @@ struct PairSolver<ANALYTIC> {
         const F2 d1 = ex2_2(fma2(lg2_2(mul2(Wn2, n1)), 1.0f / 3.0f, f2(0.528320834f)));
         F2 d = sel2(lt2(t1, f2(0.0f)), d1, d2);                                 // x < n1^2
         // (3)/(4)
-        const F2 q = mul2(n1, n2);
-        const F2 e = sub2(n3, n12);
-        const F2 z = sub2(n12, W);
-        const F2 ee = mul2(e, e);
-        const B2 c4 = is_case4_2(q, e, ee, z);
-        const F2 R = sel2(c4, fma2(q, 4.0f, mul2(ee, -1.0f)), mul2(q, 8.0f));
-        const F2 rho = rsqrt2(R);
-        const F2 K4 = mul2(mul2(mul2(q, 6.0f), sub2(n3, W)), mul2(rho, rho));
-        const F2 C = mul2(sel2(c4, K4, mul2(z, 1.5f)), rho);
-        const F2 ng = neg_sin_third_asin_fast2(C);
-        const F2 d34 = max2(fma2(mul2(R, rho), ng, sel2(c4, in.hS, n12)), n2);  // floor; drops NaN
+        const Trig34 t = trig34(in, W);
+        const F2 ng2 = neg_sin_third_asin_fast2<true>(t.C);                     // -2 g(C)
+        const F2 d34 = max2(fma2(mul2(t.R, t.rho), ng2, sel2(t.c4, in.hS, n12)), n2);   // floor; drops NaN
         d = sel2(gt2(t1, mul2(n2, sub2(n2, n1))), d34, d);                      // x > n1^2 + 3 n2 (n2 - n1)
-        return sel2(le2(n12, W), mul2(add2(W, n12), 0.5f), d);                  // (5)
+        return pair_residual(in, d, W, t.h);
     }
 };
 
 // ---------------------------------------------------------------------------------------
-// method 1, PLIC_FAST: Scardovelli-Zaleski (sect. 2.4) on a pair, branch-free: L1-normalised
-// m_i = n_i / S, alpha = d / S, thresholds multiplied through, (5) and (2) tested first, root
+// method 1, PLIC_FAST: Scardovelli-Zaleski (sect. 2.4) on a pair, branch-free: thresholds
+// multiplied through, (5) and (2) tested first, root
 //   alpha = 2 sqrt(p0) cos(acos(q0 / p0^(3/2)) / 3 + 4 pi / 3) - a2/3
 // with the collapsed p0, q0 of Precise<SZ> (plic_methods.cuh).  Micro-optimised further:
-//   * R = 4 p0 (= 8 q in case (3), 4 q - (m3 - m12)^2 in case (4)) and rho = rsqrt(R) give
-//     2 sqrt(p0) = R rho and q0 / p0^(3/2) = 8 q0 rho^3, which in case (3) is (3/2) z rho
-//     (8 q rho^2 = 1) and in case (4) 6 q (m3 - W) rho^3;
+//   * the L1 normalisation m_i = n_i / S is folded away: every quantity of the method is homogeneous
+//     in n (alpha S = d, 4 p0 S^2 = R', q0 / p0^(3/2) is scale free), so the kernel works on the n_i
+//     and never divides by S -- the precise kernel (Precise<SZ>) keeps the normalisation literally;
+//   * with R = p0 S^2 (= 2 q in case (3), u/4 in case (4)) and rho = rsqrt(R):
+//     2 sqrt(p0) S = 2 R rho and q0 / p0^(3/2) = (3/4) rho {z | q (n3 - W) rho^2}  (trig34());
 //   * the (3)-vs-(4) threshold w6 >= 6 m1 m2 m3 v3 is the sign of the case-(3)
 //     cubic at alpha = m3, a polynomial in m12 - m3 (is_case4_2), instead of the v3 polynomial;
-//   * the tests (1)/(2)/(3,4) in the scaled variable t1 = W m2 - m1^2 / 3;
+//   * the tests (1)/(2)/(3,4) in the scaled variable t1 = W n2 - n1^2 / 3;
 //   * acos by sqrt(1-x) Q5(x), the angle's 1/3 and the 4 pi / 3 in one FMA, cos on the SFU.
-// What distinguishes it from the analytic kernel is the L1 scaling (an SFU reciprocal, four
-// multiplications) and acos + cos in place of the sin(asin(.)/3) polynomial.
+// What distinguishes it from the analytic kernel is acos + cos in place of the sin(asin(.)/3)
+// polynomial.
 // ---------------------------------------------------------------------------------------
-// acos(x) for x in [0, 1] as sqrt(1-x) * Q5(x), |err| < 1.2e-6 (minimax fit,
-// fit_coefficients.py).
+// acos(x) for x in [0, 0.9] as sqrt(1-x) * Q5(x), |err| < 1.2e-6 (minimax fit on [0, 1],
+// fit_coefficients.py).  No clamps: for a cell of case (3)/(4) the argument is <= 0.884 (DESIGN.md,
+// "trig range"); elsewhere a NaN is dropped by the floor of the root.
 __device__ __forceinline__ F2 acos_fast2(F2 x) {
     F2 p = fma2(x, f2(-0.004337173733f), f2(0.01934827404f));
     p = fma2(p, x, f2(-0.04495724702f));
     p = fma2(p, x, f2(0.08787565452f));
     p = fma2(p, x, f2(-0.2145122723f));
     p = fma2(p, x, f2(1.570795206f));
-    return mul2(sqrt2(max2(fma2(x, -1.0f, f2(1.0f)), 0.0f)), p);
+    return mul2(sqrt2(fma2(x, -1.0f, f2(1.0f))), p);
 }
 
 template <>
 struct PairSolver<SZ> {
-    static __device__ __forceinline__ F2 reduced_offset(const PairIn &in) {
-        const F2 S = add2(in.n12, in.n3);
-        const F2 inv = rcp2(S);
-        const F2 m1 = mul2(in.n1, inv), m2 = mul2(in.n2, inv), m3 = mul2(in.n3, inv);
-        const F2 m12 = add2(m1, m2);
-        const F2 W = mul2(in.V2, m3);                                           // 2 w m3
-        const F2 Wm2 = mul2(W, m2);                                             // x / 3, x = 6 w m2 m3
-        const F2 s1 = mul2(m1, m1);
-        const F2 t1 = fma2(s1, -1.0f / 3.0f, Wm2);                              // (x - m1^2) / 3
-        // (2): v1 <= w <= v2, and (1): w < v1  <=>  x < m1^2;  cbrt(w6), w6 = 3 Wm2 m1
-        const F2 a2 = fma2(m1, 0.5f, sqrt2(fma2(s1, -1.0f / 12.0f, Wm2)));
-        const F2 a1 = ex2_2(fma2(lg2_2(mul2(Wm2, m1)), 1.0f / 3.0f, f2(0.528320834f)));
-        F2 alpha = sel2(lt2(t1, f2(0.0f)), a1, a2);
+    static __device__ __forceinline__ F2 residual(const PairIn &in) {
+        const F2 n1 = in.n1, n2 = in.n2, n12 = in.n12;
+        const F2 W = mul2(in.V2, in.n3);                                        // 2 w m3 S
+        const F2 Wn2 = mul2(W, n2);                                             // x S^2 / 3, x = 6 w m2 m3
+        const F2 s1 = mul2(n1, n1);
+        const F2 t1 = fma2(s1, -1.0f / 3.0f, Wn2);                              // (x - m1^2) S^2 / 3
+        // (2): v1 <= w <= v2, and (1): w < v1  <=>  x < m1^2;  alpha S = cbrt(w6 S^3), w6 S^3 = 3 Wn2 n1
+        const F2 d2 = fma2(n1, 0.5f, sqrt2(fma2(s1, -1.0f / 12.0f, Wn2)));
+        const F2 d1 = ex2_2(fma2(lg2_2(mul2(Wn2, n1)), 1.0f / 3.0f, f2(0.528320834f)));
+        F2 d = sel2(lt2(t1, f2(0.0f)), d1, d2);
         // (3)/(4)
-        const F2 q = mul2(m1, m2);
-        const F2 e = sub2(m3, m12);
-        const F2 z = sub2(m12, W);
-        const F2 ee = mul2(e, e);
-        const B2 c4 = is_case4_2(q, e, ee, z);
-        const F2 R = sel2(c4, fma2(q, 4.0f, mul2(ee, -1.0f)), mul2(q, 8.0f));  // 4 p0
-        const F2 rho = rsqrt2(R);
-        const F2 K4 = mul2(mul2(mul2(q, 6.0f), sub2(m3, W)), mul2(rho, rho));
-        const F2 arg = mul2(sel2(c4, K4, mul2(z, 1.5f)), rho);                  // q0 / p0^(3/2)
+        const Trig34 t = trig34(in, W);                                         // C = q0 / p0^(3/2)
         // cos(theta + 4 pi/3) evaluated as cos(theta - 2 pi/3): same angle, |arg| < pi
-        const F2 co = cos2(fma2(acos_fast2(min2(arg, f2(1.0f))), 1.0f / 3.0f, f2(-2.0943951f)));
-        const F2 a34 = max2(fma2(mul2(R, rho), co, sel2(c4, f2(0.5f), m12)), m2);   // floor; drops NaN
-        alpha = sel2(gt2(t1, mul2(m2, sub2(m2, m1))), a34, alpha);
-        alpha = sel2(le2(m12, W), mul2(add2(W, m12), 0.5f), alpha);             // (5)
-        return mul2(alpha, S);
+        const F2 co = cos2(fma2(acos_fast2(t.C), 1.0f / 3.0f, f2(-2.0943951f)));
+        const F2 d34 = max2(fma2(mul2(t.R, add2(t.rho, t.rho)), co, sel2(t.c4, in.hS, n12)), n2);   // floor; drops NaN
+        d = sel2(gt2(t1, mul2(n2, sub2(n2, n1))), d34, d);
+        return pair_residual(in, d, W, t.h);
     }
 };
 
 // ---------------------------------------------------------------------------------------
-// method 2, PLIC_FAST: Newton-Raphson (sect. 2.5) on a pair.  One unrolled 4-step loop on
-// F(tau) = tau^3 - p tau - r serves (1), (3) and (4) with selected (p, r, tau0, base) -- the
-// start values and trip count of Solver<NEWTON, false>, division by SFU reciprocal; every
-// lane runs it (no branch), (2) and (5) are closed forms.
+// method 2, PLIC_FAST: Newton-Raphson (sect. 2.5) on a pair.  One unrolled loop on
+// F(tau) = tau^3 - p tau - r serves (1), (3) and (4) with selected coefficients; every lane runs
+// it (no branch), (2) and (5) are closed forms, division by SFU reciprocal.
+//   * The iteration runs on sigma = -tau >= 0 with F / 2:
+//       sigma <- (sigma^3 + rn) / (3/2 sigma^2 + nh),   nh = -p/2,  rn = -r/2,
+//     one instruction less than the textbook step (no 2 tau^2); the negated form makes rn a single
+//     product: rn = (-3/2 q) {z | (n3 - W)/2}.
+//   * Start: the Newton step from tau = 0 in closed form, sigma_0 = r/p = rn / nh.  tau = 0 lies
+//     right of the root in the region where F is decreasing and concave (F(0) = -r <= 0,
+//     F' = 3 tau^2 - p < 0 on [root, 0]), so the iteration is monotone from there; 3 more steps
+//     leave 6e-8 (the round-1 kernel started at the top of the bracket and needed 4 for 4e-8).
+//   * Case (1), d^3 = 6 V n1 n2 n3 = 3 Wn2 n1: nh = 0, rn = -3/2 Wn2 n1, sigma_0 = -seed with the
+//     integer-arithmetic cube-root seed (exponent / 3), d = -sigma; 3 steps from a seed within 4 %
+//     are exact to rounding.
 // ---------------------------------------------------------------------------------------
+// start value for -cbrt(3 k3), k3 > 0: cbrt_seed() with the factor 3 folded into the constant
+// (+ lg2(3)/3 in the exponent field; 0x2a952e80 minimises the maximum relative error over
+// [1e-30, 1]: 3.9 %) and the sign bit set
+__device__ __forceinline__ float neg_cbrt3_seed(float k3) {
+    return __int_as_float((__float_as_int(k3) / 3 + 0x2a952e80) | 0x80000000);
+}
+
 template <>
 struct PairSolver<NEWTON> {
-    static __device__ __forceinline__ F2 reduced_offset(const PairIn &in) {
+    static __device__ __forceinline__ F2 residual(const PairIn &in) {
         const F2 n1 = in.n1, n2 = in.n2, n3 = in.n3, n12 = in.n12;
         const F2 W = mul2(in.V2, n3);
         const F2 Wn2 = mul2(W, n2);
-        const F2 x = mul2(Wn2, 3.0f);
         const F2 s1 = mul2(n1, n1);
-        const B2 c1 = lt2(x, s1);
+        const F2 t1 = fma2(s1, -1.0f / 3.0f, Wn2);                              // (x - n1^2) / 3
+        const B2 c1 = lt2(t1, f2(0.0f));                                        // x < n1^2
+        const B2 c34 = gt2(t1, mul2(n2, sub2(n2, n1)));                         // x > n1^2 + 3 n2 (n2 - n1)
         const F2 d2 = fma2(n1, 0.5f, sqrt2(fma2(s1, -1.0f / 12.0f, Wn2)));
         const F2 q = mul2(n1, n2);
         const F2 e = sub2(n3, n12);
         const F2 z = sub2(n12, W);
         const F2 ee = mul2(e, e);
+        const F2 h = mul2(sub2(n3, W), 0.5f);                                   // (n3 - W)/2
         const B2 c4 = is_case4_2(q, e, ee, z);
-        const F2 k = mul2(x, n1);                                               // 6 V n1 n2 n3
         const F2 zero = f2(0.0f);
-        // F / 2: the iteration tau <- (tau^3 + r/2) / (3/2 tau^2 - p/2) is the Newton step with
-        // one instruction less (no 2 tau^2); nh = -p/2, rh = r/2
-        F2 nh = sel2(c4, mul2(fma2(q, 4.0f, mul2(ee, -1.0f)), -0.375f), mul2(q, -3.0f));
-        F2 rh = mul2(q, sel2(c4, mul2(sub2(n3, W), 0.75f), mul2(z, 1.5f)));
-        F2 tau = sel2(c4, zero, min2(e, zero));
-        F2 base = sel2(c4, in.hS, n12);
-        nh = sel2(c1, zero, nh);
-        rh = sel2(c1, mul2(k, 0.5f), rh);
-        tau = sel2(c1, F2{cbrt_seed(k.x), cbrt_seed(k.y)}, tau);
-        base = sel2(c1, zero, base);
-        const F2 floor_ = sel2(c1, zero, n2);
+        const F2 qm = mul2(q, -1.5f);
+        const F2 nh34 = sel2(c4, fma2(ee, 0.375f, qm), add2(qm, qm));           // -3u/8 | -3q
+        const F2 rn34 = mul2(qm, sel2(c4, h, z));                               // -3/4 q (n3 - W) | -3/2 q z
+        const F2 k3 = mul2(Wn2, n1);                                            // 2 V n1 n2 n3
+        const F2 nh = sel2(c1, zero, nh34);
+        const F2 rn = sel2(c1, mul2(k3, -1.5f), rn34);
+        F2 sig = sel2(c1, F2{neg_cbrt3_seed(k3.x), neg_cbrt3_seed(k3.y)}, mul2(rn34, rcp2(nh34)));
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const F2 t2 = mul2(tau, tau);
-            tau = mul2(fma2(t2, tau, rh), rcp2(fma2(t2, 1.5f, nh)));
+        for (int i = 0; i < 3; ++i) {
+            const F2 s2 = mul2(sig, sig);
+            sig = mul2(fma2(s2, sig, rn), rcp2(fma2(s2, 1.5f, nh)));
         }
-        const F2 dn = max2(add2(base, tau), floor_);                            // floor; drops NaN
-        const F2 thr = fma2(mul2(n2, 3.0f), sub2(n2, n1), s1);
-        const B2 it = B2{c1.x || x.x > thr.x, c1.y || x.y > thr.y};
-        const F2 d = sel2(it, dn, d2);
-        return sel2(le2(n12, W), mul2(add2(W, n12), 0.5f), d);                  // (5)
+        const F2 d34 = max2(fma2(sig, -1.0f, sel2(c4, in.hS, n12)), n2);        // floor; drops NaN
+        F2 d = sel2(c34, d34, d2);
+        d = sel2(c1, F2{-sig.x, -sig.y}, d);
+        return pair_residual(in, d, W, h);
     }
 };
 
@@ -339,7 +367,7 @@ struct NestedSteps<N, N> {
 
 template <>
 struct PairSolver<NESTED> {
-    static __device__ __forceinline__ F2 reduced_offset(const PairIn &in) {
+    static __device__ __forceinline__ F2 residual(const PairIn &in) {
         const F2 n1 = in.n1, n2 = in.n2, n3 = in.n3, n12 = in.n12;
         const F2 W = mul2(in.V2, n3);
         const F2 Wn2 = mul2(W, n2);                                             // x / 3
@@ -352,10 +380,12 @@ struct PairSolver<NESTED> {
         const F2 e = sub2(n3, n12);
         const F2 z = sub2(n12, W);
         const F2 ee = mul2(e, e);
+        const F2 h = mul2(sub2(n3, W), 0.5f);                                   // (n3 - W)/2
         const B2 c4 = is_case4_2(q, e, ee, z);
         const F2 zero = f2(0.0f);
-        const F2 np = sel2(c4, mul2(fma2(q, 4.0f, mul2(ee, -1.0f)), -0.75f), mul2(q, -6.0f));   // -p
-        const F2 nr = mul2(q, sel2(c4, mul2(sub2(n3, W), -1.5f), mul2(z, -3.0f)));              // -r
+        const F2 qm = mul2(q, -3.0f);
+        const F2 np = sel2(c4, fma2(ee, 0.75f, qm), add2(qm, qm));              // -p: -3u/4 | -6q
+        const F2 nr = mul2(qm, sel2(c4, h, z));                                 // -r: -3/2 q (n3 - W) | -3 q z
         const F2 lo = sel2(c4, sub2(n3, in.hS), mul2(n1, -1.0f));
         const F2 hi = sel2(c4, zero, min2(e, zero));
         const F2 w = sub2(hi, lo);
@@ -367,7 +397,7 @@ struct PairSolver<NESTED> {
         NestedSteps<0, 20>::run(c, nP, nR, sign_mask_register());
         const F2 d34 = max2(fma2(c, w, sel2(c4, in.hS, n12)), n2);              // floor; drops NaN
         d = sel2(gt2(t1, mul2(n2, sub2(n2, n1))), d34, d);
-        return sel2(le2(n12, W), mul2(add2(W, n12), 0.5f), d);                  // (5)
+        return pair_residual(in, d, W, h);
     }
 };
 
@@ -375,7 +405,7 @@ struct PairSolver<NESTED> {
 template <int METHOD>
 __device__ __forceinline__ F2 solve_pair_fast(F2 V0, F2 nx, F2 ny, F2 nz) {
     const PairIn in = pair_reduce(V0, nx, ny, nz);
-    return pair_restore(V0, in.hS, PairSolver<METHOD>::reduced_offset(in));
+    return pair_restore(V0, PairSolver<METHOD>::residual(in));
 }
 
 // ---------------------------------------------------------------------------------------
@@ -469,7 +499,7 @@ __device__ __forceinline__ F2 sphere_volume_pair(F2 d0) {
 
 __device__ __forceinline__ F2 sphere_solve_pair_fast(F2 V0) {
     const F2 V = sat2(min2(V0, fma2(V0, -1.0f, f2(1.0f))));
-    const F2 nsin = neg_sin_third_asin_fast2(sqrt2(V));                          // -sin(psi)
+    const F2 nsin = neg_sin_third_asin_fast2<false>(sqrt2(V));                          // -sin(psi)
     const F2 cosp = sqrt2(fma2(mul2(nsin, -1.0f), nsin, f2(1.0f)));              // cos(psi)
     // a = 4r sin(psi) (sqrt(3)/2 cos(psi) + 1/2 sin(psi))
     const F2 a = mul2(mul2(nsin, -4.0f * kSphereR), fma2(cosp, 0.866025404f, mul2(nsin, -0.5f)));
