@@ -275,7 +275,8 @@ struct PairSolver<SZ> {
 // (+ lg2(3)/3 in the exponent field; 0x2a952e80 minimises the maximum relative error over
 // [1e-30, 1]: 3.9 %) and the sign bit set
 __device__ __forceinline__ float neg_cbrt3_seed(float k3) {
-    return __int_as_float((__float_as_int(k3) / 3 + 0x2a952e80) | 0x80000000);
+    // k3 >= 0: unsigned high multiply = bits / 3 (one IMAD.HI, no sign fix-up)
+    return __uint_as_float((__umulhi(__float_as_uint(k3), 0x55555556u) + 0x2a952e80u) | 0x80000000u);
 }
 
 template <>
