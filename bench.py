@@ -309,14 +309,36 @@ def profile_table(name):
     return rows
 
 
+def csrc_digest():
+    """sha1 (12 hex digits) over the kernel sources with comments and white space removed: the
+    committed ncu tables carry the digest they were captured at, so a table that no longer matches
+    the kernels' code is reported as stale instead of silently reused."""
+    import glob
+    import hashlib
+    import re
+    h = hashlib.sha1()
+    src = os.path.join(ROOT, "paper_2006_12838_b200", "csrc")
+    for f in sorted(glob.glob(os.path.join(src, "*.cu")) + glob.glob(os.path.join(src, "*.cuh"))):
+        with open(f, "r", encoding="utf-8", errors="replace") as fh:
+            code = re.sub(r"/\*.*?\*/", "", fh.read(), flags=re.S)
+        code = re.sub(r"//[^\n]*", "", code)
+        h.update(os.path.basename(f).encode() + b"\0" + re.sub(r"\s+", "", code).encode())
+    return h.hexdigest()[:12]
+
+
+def table_is_stale(table):
+    return table.get("@csrc_sha1", ["?"])[0] != csrc_digest()
+
+
 def ncu_traffic(kernel_name, cells):
     """(dram bytes per launch, provenance) of `kernel_name` from the committed ncu capture -- only
     when that capture was taken on the same number of cells, else (None, why)."""
     t = profile_table("dram_traffic.txt")
     row = t.get(kernel_name)
     cap_cells = int(t.get("@cells", ["0"])[0])
-    src = "profiles/dram_traffic.txt (ncu --set full, commit %s, %d cells per launch)" % (
-        t.get("@commit", ["?"])[0], cap_cells)
+    src = "profiles/dram_traffic.txt (ncu --set full, commit %s, %d cells per launch%s)" % (
+        t.get("@commit", ["?"])[0], cap_cells,
+        "; STALE: the kernel sources changed since this capture" if table_is_stale(t) else "")
     if row is None:
         return None, "no ncu capture of this kernel in profiles/dram_traffic.txt"
     if cap_cells != cells:
@@ -751,7 +773,10 @@ def run_ours(args):
                     "api": "plic_solve_host (pinned host arrays, chunked H2D/kernel/D2H pipeline inside libplic)",
                     "timer": "host wall clock around the synchronous calls, device synchronised on both sides"},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "kernel": head,
+                         "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
+                         "tables_stale": {"dram_traffic.txt": table_is_stale(profile_table("dram_traffic.txt")),
+                                          "instruction_counts.txt": table_is_stale(counts)},
+                         "kernel": head,
                          "frac_nominal": achieved / NOMINAL_HBM_GBS, "peak_nominal": NOMINAL_HBM_GBS,
                          "frac_of_stream_ceiling": stream_ceiling["ms_per_step"] / H["ms_per_step"],
                          "issue_frac": H.get("issue_frac"),

@@ -1,12 +1,14 @@
 // plic_packed.cuh -- two cells per instruction: packed fp32x2 arithmetic (sm_100a).
 //
 // Blackwell adds add/mul/fma on a pair of fp32 values held in one 64-bit register pair
-// (PTX add.f32x2 / mul.f32x2 / fma.rn.f32x2, SASS FADD2 / FMUL2 / FFMA2).  One issue slot then
-// carries the arithmetic of two cells.  The PLIC kernels are bound by instruction issue, not
-// by a single pipe (profiles/r01_ncu_summary.md: issue-active 78 %, fma 46 %, alu 44 %, xu
-// 35 %), and about half of their instructions are plain mul/add/fma, so the branch-free
-// variants run on pairs: every mul/add/fma is packed, while min/max/compare/select and the
-// SFU ops, which have no packed form, are issued per half.
+// (PTX add.f32x2 / mul.f32x2 / fma.rn.f32x2, SASS FADD2 / FMUL2 / FFMA2).  About half the
+// instructions of a branch-free PLIC method are plain mul/add/fma, so the PLIC_FAST variants run
+// on pairs: every mul/add/fma is packed, while min/max/compare/select and the SFU ops, which
+// have no packed form, are issued per half.  A packed instruction halves the instruction count
+// of that arithmetic but holds the issue port for two clocks (plic_probe.cuh: FFMA2 0.50 per
+// clock, FFMA2 + LOP3 0.66 = three clocks per pair), so the ceiling of these kernels is counted
+// in issue slots = instructions + packed instructions; what packing buys
+// is registers, instruction-cache and scoreboard pressure.
 //
 // F2 is a plain pair of floats.  mov.b64 {lo,hi} in the helpers only names the register
 // pair; ptxas allocates both halves adjacent and emits no move for it.
@@ -139,9 +141,12 @@ __device__ __forceinline__ F2 pair_residual(const PairIn &in, F2 d, F2 W, F2 h) 
 }
 
 // A-priori (3)-vs-(4) decision on a pair: case (4) iff n3 < n12 and F3(e) > 0 (is_case4()).
-__device__ __forceinline__ B2 is_case4_2(F2 q, F2 e, F2 ee, F2 z) {
-    const F2 h = fma2(fma2(q, -6.0f, ee), e, mul2(mul2(q, z), -3.0f));
-    return B2{e.x < 0.0f && h.x > 0.0f, e.y < 0.0f && h.y > 0.0f};
+// With z = n12 - W and e = n3 - n12, z + 2e = (n3 - W) + e, so
+//   F3(e) = e^3 - 6 q e - 3 q z = e^3 - 3 q e - 3 q (n3 - W) = -3 [ q (n3 - W) + e (q - e^2/3) ],
+// two FMAs on qn = q (n3 - W), which the case-(4) root needs anyway.
+__device__ __forceinline__ B2 is_case4_2(F2 q, F2 e, F2 ee, F2 qn) {
+    const F2 h = fma2(e, fma2(ee, -1.0f / 3.0f, q), qn);                         // -F3(e) / 3
+    return B2{e.x < 0.0f && h.x < 0.0f, e.y < 0.0f && h.y < 0.0f};
 }
 
 template <int METHOD>
@@ -172,11 +177,12 @@ __device__ __forceinline__ Trig34 trig34(const PairIn &in, F2 W) {
     const F2 z = sub2(in.n12, W);
     const F2 ee = mul2(e, e);
     const F2 n3mW = sub2(in.n3, W);
+    const F2 qn = mul2(q, n3mW);
     t.h = mul2(n3mW, 0.5f);
-    t.c4 = is_case4_2(q, e, ee, z);
+    t.c4 = is_case4_2(q, e, ee, qn);
     t.R = sel2(t.c4, fma2(ee, -0.25f, q), add2(q, q));                          // u/4 | 2 q
     t.rho = rsqrt2(t.R);
-    const F2 K4 = mul2(mul2(q, n3mW), mul2(t.rho, t.rho));
+    const F2 K4 = mul2(qn, mul2(t.rho, t.rho));
     t.C = mul2(sel2(t.c4, K4, z), mul2(t.rho, 0.75f));
     return t;
 }
@@ -294,8 +300,9 @@ struct PairSolver<NEWTON> {
         const F2 e = sub2(n3, n12);
         const F2 z = sub2(n12, W);
         const F2 ee = mul2(e, e);
-        const F2 h = mul2(sub2(n3, W), 0.5f);                                   // (n3 - W)/2
-        const B2 c4 = is_case4_2(q, e, ee, z);
+        const F2 n3mW = sub2(n3, W);
+        const F2 h = mul2(n3mW, 0.5f);                                          // (n3 - W)/2
+        const B2 c4 = is_case4_2(q, e, ee, mul2(q, n3mW));
         const F2 zero = f2(0.0f);
         const F2 qm = mul2(q, -1.5f);
         const F2 nh34 = sel2(c4, fma2(ee, 0.375f, qm), add2(qm, qm));           // -3u/8 | -3q
@@ -381,8 +388,9 @@ struct PairSolver<NESTED> {
         const F2 e = sub2(n3, n12);
         const F2 z = sub2(n12, W);
         const F2 ee = mul2(e, e);
-        const F2 h = mul2(sub2(n3, W), 0.5f);                                   // (n3 - W)/2
-        const B2 c4 = is_case4_2(q, e, ee, z);
+        const F2 n3mW = sub2(n3, W);
+        const F2 h = mul2(n3mW, 0.5f);                                          // (n3 - W)/2
+        const B2 c4 = is_case4_2(q, e, ee, mul2(q, n3mW));
         const F2 zero = f2(0.0f);
         const F2 qm = mul2(q, -3.0f);
         const F2 np = sel2(c4, fma2(ee, 0.75f, qm), add2(qm, qm));              // -p: -3u/4 | -6q
