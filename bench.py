@@ -645,7 +645,7 @@ def run_ours(args):
                    "cells": N4, "generator_s": gen_s, "methods": r4}
         del a4, o4
 
-    # ---- curvature on configs[4]: 256^3 lattice, sphere R = 60 (sect. 4; two launches per call) ----
+    # ---- curvature on configs[4]: 256^3 lattice, sphere R = 60 (sect. 4; three launches per call) ----
     curv = None
     if not args.no_curvature:
         R5 = 60.0

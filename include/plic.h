@@ -218,10 +218,10 @@ int plic_sphere_volume(const float *d0, float *V0, int64_t N, cudaStream_t strea
  * a lone neighbour, neighbours on one line or coplanar with the normal, coincident abscissae) is
  * dropped like the parameters beyond the number of points: it stays 0 and takes no part
  * in the elimination.  kappa is therefore finite for every finite lattice.
- * A 4-byte memset and two kernels are enqueued on `stream`: a streaming pass (128-bit accesses when phi
- * and kappa are 16-byte aligned, scalar otherwise) and, as a programmatic dependent launch, a dense pass
- * over the interface list with two lanes per point.  Aligned and unaligned calls give bitwise the same
- * kappa.  Errors, ownership and stream semantics as plic_solve.
+ * Three kernels are enqueued on `stream`, each a programmatic dependent launch of its predecessor: the
+ * reset of the list counter, a streaming pass (128-bit accesses when phi and kappa are 16-byte aligned,
+ * scalar otherwise) and a dense pass over the interface list, one thread per point.  Aligned and
+ * unaligned calls give bitwise the same kappa.  Errors, ownership and stream semantics as plic_solve.
  */
 int plic_curvature(const float *phi, float *kappa, int nx, int ny, int nz, int32_t *work,
                    int64_t work_entries, cudaStream_t stream);

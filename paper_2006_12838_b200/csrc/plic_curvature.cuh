@@ -44,12 +44,22 @@ __device__ __forceinline__ bool curv_interior(int64_t i, int nx, int ny, int nz)
     return x > 0 && x < nx - 1 && y > 0 && y < ny - 1 && z > 0 && z < nz - 1;
 }
 
+// ---- curv_reset ----------------------------------------------------------------------------
+// Clears the list counter.  A kernel (not a memset) so that the three launches of a call form one
+// chain of programmatic dependent launches: each becomes resident while its predecessor drains and
+// touches global memory only after griddepcontrol.wait, i.e. after the predecessor has completed.
+__global__ void curv_reset(int *__restrict__ list) {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (threadIdx.x == 0) list[0] = 0;
+}
+
 // ---- curv_mark -----------------------------------------------------------------------------
 // list[0] counts every interior interface point found (also beyond capacity); entries
 // list[1 .. min(count, capacity)] hold linear cell indices x + nx (y + ny z).
 __global__ void __launch_bounds__(256)
 curv_mark(const float *__restrict__ phi, float *__restrict__ kappa, int nx, int ny, int nz,
           int *__restrict__ list, int capacity) {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int64_t ncells = (int64_t)nx * ny * nz;
     const int64_t stride = (int64_t)gridDim.x * 256;
     const int lane = threadIdx.x & 31;
@@ -137,6 +147,7 @@ curv_mark4(const float4 *__restrict__ phi, float4 *__restrict__ kappa, int nx, i
     __shared__ MarkShared sh;
     if (threadIdx.x == 0) sh.count = 0;
     __syncthreads();
+    asm volatile("griddepcontrol.wait;" ::: "memory");           // before the first global access
     // whole warps iterate together (the append uses warp collectives): bound by the warp's first lane
     for (int64_t base = (int64_t)blockIdx.x * 256 + (threadIdx.x & ~31); base < n4;
          base += kMarkGroups * stride) {
@@ -333,15 +344,18 @@ curv_cells(const float *__restrict__ phi, float *__restrict__ kappa, int nx, int
     // launched with programmatic stream serialization: the blocks may become resident while
     // curv_mark drains; nothing of its output is read before this wait
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    const int found = list[0];
-    const int count = found < capacity ? found : capacity;
-    const int64_t sy = nx, sz = (int64_t)nx * ny;
     const int sub = threadIdx.x % kPointLanes;
     const int per = kCurvBlock / kPointLanes;
+    // the count and this thread's first list entry are independent loads: one memory round trip, not two
+    const int jfirst = blockIdx.x * per + threadIdx.x / kPointLanes;
+    const int found = list[0];
+    int cfirst = list[1 + (jfirst < capacity ? jfirst : 0)];        // capacity >= 1; stale beyond the count, unused then
+    const int count = found < capacity ? found : capacity;
+    const int64_t sy = nx, sz = (int64_t)nx * ny;
     for (int j0 = blockIdx.x * per; j0 < count; j0 += gridDim.x * per) {     // uniform per block
         const int j = j0 + threadIdx.x / kPointLanes;
         const bool live = j < count;
-        const int64_t c = list[1 + (live ? j : count - 1)];
+        const int64_t c = (j == jfirst && live) ? cfirst : list[1 + (live ? j : count - 1)];
         const float k = curvature_point<kPointLanes>(phi, c, sy, sz, sub);
         if (live && sub == 0) kappa[c] = k;
     }

@@ -802,35 +802,43 @@ int plic_curvature(const float *phi, float *kappa, int nx, int ny, int nz, int32
     int64_t cap64 = work_entries - 1;
     if (cap64 > ncells) cap64 = ncells;
     const int capacity = (int)cap64;
-    if (cudaMemsetAsync(work, 0, sizeof(int32_t), stream) != cudaSuccess) return PLIC_ERR_LAUNCH;
+    // three launches, each a programmatic dependent launch of its predecessor: the launch latencies
+    // hide behind the preceding kernel's tail; every kernel waits (griddepcontrol.wait) before its
+    // first global access
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cfg.gridDim = dim3(1);
+    cfg.blockDim = dim3(32);
+    if (cudaLaunchKernelEx(&cfg, plic::curv_reset, (int *)work) != cudaSuccess) return PLIC_ERR_LAUNCH;
     int64_t need, full = (int64_t)info->sms * 8;
+    cfg.blockDim = dim3(256);
     if ((((uintptr_t)phi | (uintptr_t)kappa) & 15u) == 0 && ncells >= 4) {
         need = (ncells / 4 + 256 * plic::kMarkGroups - 1) / (256 * plic::kMarkGroups);
-        plic::curv_mark4<<<(int)need, 256, 0, stream>>>(
-            (const float4 *)phi, (float4 *)kappa, nx, ny, nz, work, capacity);
+        cfg.gridDim = dim3((unsigned)need);
+        if (cudaLaunchKernelEx(&cfg, plic::curv_mark4, (const float4 *)phi, (float4 *)kappa, nx, ny, nz,
+                               (int *)work, capacity) != cudaSuccess)
+            return PLIC_ERR_LAUNCH;
     } else {
         need = (ncells + 255) / 256;
-        plic::curv_mark<<<(int)(need < full ? need : full), 256, 0, stream>>>(phi, kappa, nx, ny, nz,
-                                                                             work, capacity);
+        cfg.gridDim = dim3((unsigned)(need < full ? need : full));
+        if (cudaLaunchKernelEx(&cfg, plic::curv_mark, phi, kappa, nx, ny, nz, (int *)work, capacity) !=
+            cudaSuccess)
+            return PLIC_ERR_LAUNCH;
     }
     need = ((int64_t)capacity * plic::kPointLanes + plic::kCurvBlock - 1) / plic::kCurvBlock;
     full = (int64_t)info->sms * 16;
-    {   // programmatic dependent launch: hides the launch latency behind the tail of the marking pass
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)(need < full ? need : full));
-        cfg.blockDim = dim3(plic::kCurvBlock);
-        cfg.dynamicSmemBytes = 0;
-        cfg.stream = stream;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        attr[0].val.programmaticStreamSerializationAllowed = 1;
-        cfg.attrs = attr;
-        cfg.numAttrs = 1;
-        const int *list = work;
-        if (cudaLaunchKernelEx(&cfg, plic::curv_cells, phi, kappa, nx, ny, list, capacity) != cudaSuccess)
-            return PLIC_ERR_LAUNCH;
-    }
-    plic::g_launches.fetch_add(2, std::memory_order_relaxed);
+    cfg.gridDim = dim3((unsigned)(need < full ? need : full));
+    cfg.blockDim = dim3(plic::kCurvBlock);
+    const int *list = work;
+    if (cudaLaunchKernelEx(&cfg, plic::curv_cells, phi, kappa, nx, ny, list, capacity) != cudaSuccess)
+        return PLIC_ERR_LAUNCH;
+    plic::g_launches.fetch_add(3, std::memory_order_relaxed);
     return cudaPeekAtLastError() == cudaSuccess ? PLIC_OK : PLIC_ERR_LAUNCH;
 }
 

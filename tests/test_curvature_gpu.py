@@ -42,7 +42,7 @@ def run_gpu(plic, phi, work_entries=None):
         work = torch.empty(1 + t.numel(), dtype=torch.int32, device="cuda")
     k = plic.plic_curvature(t, work=work)
     torch.cuda.synchronize()
-    assert plic.plic_launch_count() == before + 2          # streaming pass + pass over the interface list
+    assert plic.plic_launch_count() == before + 3          # counter reset + streaming pass + pass over the interface list
     return k.cpu().numpy(), work.cpu().numpy()
 
 
