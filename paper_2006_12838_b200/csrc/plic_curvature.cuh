@@ -210,6 +210,9 @@ __device__ __forceinline__ float curvature_point(const float *__restrict__ phi, 
     const float *pc = phi + c;
     const int isy = (int)sy, isz = (int)sz;                          // ncells < 2^31
     float g[3] = {0.0f, 0.0f, 0.0f};
+#if PLIC_CURV_KEEP
+    float keep_p[SLOTS], keep_m[SLOTS];
+#endif
     // step 1: eq. (54), weights eq. (55): 4, 2, 1 for |e|_1 = 1, 2, 3; the pair contributes w e (phi+ - phi-).
     // The fill levels are not kept: step 3 reads them again (L1 hits), which frees ~35 registers.
 #pragma unroll
@@ -219,7 +222,13 @@ __device__ __forceinline__ float curvature_point(const float *__restrict__ phi, 
         const int ex = k - 3 * t - 1, ey = t - (t >= 3 ? 3 : 0) - 1, ez = (k >= 9 ? 1 : 0) - 1;
         const int off = ex + ey * isy + ez * isz;
         const int l1 = (ex != 0) + (ey != 0) + (ez != 0);
+#if PLIC_CURV_KEEP
+        keep_p[s] = __ldg(pc + off);
+        keep_m[s] = __ldg(pc - off);
+        const float w = k < 13 ? (float)(8 >> l1) * (keep_p[s] - keep_m[s]) : 0.0f;
+#else
         const float w = k < 13 ? (float)(8 >> l1) * (__ldg(pc + off) - __ldg(pc - off)) : 0.0f;
+#endif
         g[0] = fmaf(w, (float)ex, g[0]);
         g[1] = fmaf(w, (float)ey, g[1]);
         g[2] = fmaf(w, (float)ez, g[2]);
@@ -254,7 +263,11 @@ __device__ __forceinline__ float curvature_point(const float *__restrict__ phi, 
         const int t = (k * 11) >> 5;
         const int ex = k - 3 * t - 1, ey = t - (t >= 3 ? 3 : 0) - 1, ez = (k >= 9 ? 1 : 0) - 1;
         const int off = ex + ey * isy + ez * isz;
+#if PLIC_CURV_KEEP
+        const float pp = keep_p[s], pm = keep_m[s];
+#else
         const float pp = __ldg(pc + off), pm = __ldg(pc - off);
+#endif
         const F2 d0 = solve_pair_fast<ANALYTIC>(F2{pp, pm}, NX, NY, NZ);
         if (q == 0) d00 = LANES == 1 ? d0.x : __shfl_sync(full, d0.x, (threadIdx.x & (32 - LANES)) | 1);   // from lane sub = 1
         const bool u0 = k < 13 && pp > 0.0f && pp < 1.0f, u1 = k < 13 && pm > 0.0f && pm < 1.0f;
@@ -326,6 +339,9 @@ __device__ __forceinline__ float curvature_point(const float *__restrict__ phi, 
 }
 
 // ---- curv_cells: kPointLanes lanes per entry of the caller's list ------------------------------------
+#ifndef PLIC_CURV_KEEP
+#define PLIC_CURV_KEEP 1     // keep the 26 fill levels in registers between step 1 and step 3 (0: read them again, L1 hits)
+#endif
 #ifndef PLIC_CURV_LANES
 #define PLIC_CURV_LANES 1
 #endif

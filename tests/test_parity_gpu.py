@@ -337,6 +337,35 @@ def test_full_size_config2_sampled(plic):
         assert float((back - tV).abs().max()) <= 2e-5                          # eq. (31)
 
 
+def test_full_size_config3_sampled(plic):
+    """configs[2] at its full size, in the layouts bench.py's `divergence` leg times: N = 2^26 cells
+    labelled by the oracle, 20 % per intersection case, interleaved (every warp holds all five cases) and
+    gathered into five case-contiguous blocks.  Properties on every cell, the oracle on every 64th cell
+    with the error per case; both layouts hold the same cells, so their results agree bitwise after the
+    gather."""
+    N = 1 << 26
+    V0, nx, ny, nz, kase = stratified(N, seed=2)
+    assert np.all(np.abs(np.bincount(kase, minlength=6)[1:] - N / 5) <= 1)
+    order = np.concatenate([np.arange(k, N, 5) for k in range(5)])
+    sl = slice(3, None, 64)
+    ref = oracle.solve(V0[sl], nx[sl], ny[sl], nz[sl])
+    tV, tx, ty, tz = dev(V0, nx, ny, nz)
+    torder = torch.from_numpy(order).cuda()
+    cV, cx, cy, cz = [t[torder].contiguous() for t in (tV, tx, ty, tz)]
+    S2 = 0.5 * (tx.abs() + ty.abs() + tz.abs())
+    out, outc = torch.empty_like(tV), torch.empty_like(tV)
+    for method, fast in VARIANTS:
+        plic.plic_solve(tV, tx, ty, tz, out=out, method=method, fast=fast)
+        plic.plic_solve(cV, cx, cy, cz, out=outc, method=method, fast=fast)
+        assert bool(torch.isfinite(out).all()) and bool((out.abs() <= S2 * (1 + 1e-6)).all())
+        assert bool(torch.equal(out[torder], outc)), (method, fast)              # layout independent
+        err = np.abs(out[sl].cpu().numpy().astype(np.float64) - ref)
+        for k in range(1, 6):
+            assert err[kase[sl] == k].max() <= TOL_D0, (method, fast, k)
+        back = plic.plic_volume(out, tx, ty, tz)
+        assert float((back - tV).abs().max()) <= 2e-5                          # eq. (31)
+
+
 def test_full_size_config4_sampled(plic):
     """configs[3]: N = 2^28 cells (4.3 GB in, 1.1 GB out), half the normals snapped to an axis or a
     face diagonal, V0 ~ Beta(1/2, 1/2): properties on every cell, the oracle on every 1024th."""
