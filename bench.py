@@ -22,7 +22,9 @@ Per method: `hbm_frac` against the measured copy bandwidth and `h
 against 8 TB/s; `issue_frac` = issue slots per cell x cells/s / (SMs x 4 sub-partitions x the SM
 clock sampled in that method's timed window), issue slots = warp-instructions (ncu's executed count)
 + packed fp32x2 warp-instructions (they hold the issue port for two clocks, see pipe_rates), both per
-cell from the committed table profiles/instruction_counts.txt; `bound` names the larger fraction.  "stream_ceiling" is the
+cell from the committed table profiles/instruction_counts.txt; `bound` names the larger fraction;
+`issue_frac_algorithmic` is the same from SURVEY.md 8d's algorithmic operation counts (union of all case
+paths) against SMs x 128 FP32 lanes x clock.  "stream_ceiling" is the
 same 4-read/1-write stream with no arithmetic (plic_solve with the blank method, d0 = V0 - 1/2);
 "pipe_rates" are the instruction rates of the FMA, SFU and ALU pipes measured in this run
 (plic_pipe_probe), from which the "alu" peak of the compute-bound legs is derived.
@@ -381,6 +383,8 @@ def pcie_link(sampler):
 
 
 VARIANTS = [(m, f) for f in (True, False) for m in ("analytic", "sz", "newton", "nested")]
+# SURVEY.md 8d, "Algorithmic work per cell": FP32 + SFU operations of the union of all case paths
+ALGORITHMIC_INST = {"analytic": 95 + 7, "sz": 95 + 7, "newton": 105 + 8, "nested": 190 + 3}
 
 
 def time_variants(plic, arrays, out, steps, warmup, stream, world, sampler, sms, counts, peak):
@@ -401,6 +405,12 @@ def time_variants(plic, arrays, out, steps, warmup, stream, world, sampler, sms,
              "hbm_frac_nominal": gbs / NOMINAL_HBM_GBS, "sm_mhz": clk.get("sm_mhz")}
         e["roofline_frac"] = e["hbm_frac"]
         issue_fields(e, counts.get(name), N, ms, sms, clk.get("sm_mhz"))
+        if clk.get("sm_mhz"):
+            # SURVEY.md 8d also asks for the issue fraction from the ALGORITHMIC counts: the thread-
+            # instructions per cell a mixed warp has to issue for the method's formulas (union of all
+            # case paths, SURVEY.md 8d "Algorithmic work per cell"), against SMs x 128 lanes x clock
+            e["algorithmic_thread_inst_per_cell"] = ALGORITHMIC_INST[m]
+            e["issue_frac_algorithmic"] = ALGORITHMIC_INST[m] * N / (ms * 1e-3) / (sms * 128 * clk["sm_mhz"] * 1e6)
         res[name] = e
     return res
 

@@ -13,20 +13,23 @@
 //
 // Interface points are a 2-D surface in a 3-D lattice (0.4 % of the cells of a 256^3 box holding an
 // R = 60 drop), so a thread per lattice cell would run the ~2000-instruction point routine in warps
-// with one or two active lanes.  Two kernels instead:
+// with one or two active lanes.  Two passes instead (three launches per call, chained as programmatic
+// dependent launches; curv_reset clears the list counter first):
 //   curv_mark4  streams the lattice once (HBM bound: 4 B read + 4 B written per cell), writes
 //               kappa = 0 everywhere and collects the interior interface points per block in shared
 //               memory (warp-aggregated), flushed to the caller's list with one global atomicAdd per
 //               block; curv_mark is its scalar form for lattices off the 16-byte boundary;
-//   curv_cells  the list entries in dense warps, kPointLanes LANES PER POINT: the 13 neighbour pairs
-//               (e, -e) and the centre are dealt to the lanes of a point, which gather their fill
-//               levels (L2 hits, the lattice has just been streamed), solve their PLIC offsets with the
-//               packed analytic solver and accumulate their share of the 17 moments; gradient sums and
-//               moments are reduced with xor shuffles.  One thread per point (round 1) left 3 warps per
-//               SM sub-partition with a 2000-instruction dependent chain each: latency bound at 16 %
-//               occupancy.  (Evaluating the points inside the streaming kernel -- each block its own
-//               -- was tried: 49 us per call instead of 38, the point routine's registers cut the
-//               streaming occupancy and every block with a single point pays a full round.)
+//   curv_cells  the list entries in dense warps, kPointLanes lanes per point (1 by default; 2 and 4 are
+//               kept as template instances: the 13 neighbour pairs (e, -e) and the centre are dealt to
+//               the lanes of a point, gradient sums and moments reduced with xor shuffles).  A lane
+//               gathers its fill levels (L2 hits, the lattice has just been streamed), solves its PLIC
+//               offsets with the packed analytic solver and accumulates its share of the 17 moments.
+//               Measured on the 256^3 / R = 60 lattice: every split that keeps
+//               the registers is equal within 0.2 us -- more lanes shorten one point's dependent chain
+//               but add waves -- so the pass is bound by one point's latency, not by throughput.
+//               (Evaluating the points inside the streaming kernel -- each block its own -- was tried:
+//               49 us per call instead of 38, the point routine's registers cut the streaming
+//               occupancy and every block with a single point pays a full round.)
 // Readings C1-C5 of oracle/curvature.py's header apply (sign of kappa, zero for non-interface /
 // border / gradient-free / neighbour-free points, reduced rank keeps the first k parameters).
 #pragma once
