@@ -366,6 +366,36 @@ def test_full_size_config3_sampled(plic):
         assert float((back - tV).abs().max()) <= 2e-5                          # eq. (31)
 
 
+def test_more_than_2_31_cells(plic):
+    """Maximum sizes: N = 2^31 + 2^20 + 5 cells (8.6 GB per array), beyond 32-bit element indices and with
+    a ragged tail.  The input is a 2^22-cell block of configs[1] tiled on the device, so the expected
+    output is the block's own result tiled: compared bitwise, chunk by chunk, for one kernel of each
+    streaming body (map_tma, map_vec4, map_compact) and plic_volume.  Skipped when the device has less
+    than 60 GB free."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 60 * (1 << 30):
+        pytest.skip("needs 60 GB of free device memory")
+    B = 1 << 22
+    N = (1 << 31) + (1 << 20) + 5
+    reps = (N + B - 1) // B
+    base = dev(*gen.random_sphere(B, seed=1))
+    big = [t.repeat(reps)[:N].contiguous() for t in base]
+    out = torch.empty(N, dtype=torch.float32, device="cuda")
+    for method, fast in (("analytic", True), ("nested", True), ("analytic", False)):
+        want = plic.plic_solve(*base, method=method, fast=fast)
+        out.fill_(float("nan"))
+        plic.plic_solve(*big, out=out, method=method, fast=fast)
+        full = (N // B) * B
+        assert bool(torch.equal(out[:full].view(-1, B), want.expand(N // B, B))), (method, fast)
+        assert bool(torch.equal(out[full:], want[:N - full])), (method, fast)
+    want = plic.plic_volume(base[0], *base[1:])                  # any d0 in range will do: reuse V0 as d0
+    plic.plic_volume(big[0], *big[1:], out=out)
+    assert bool(torch.equal(out[:(N // B) * B].view(-1, B), want.expand(N // B, B)))
+    assert bool(torch.equal(out[(N // B) * B:], want[:N - (N // B) * B]))
+    del big, out
+    torch.cuda.empty_cache()
+
+
 def test_full_size_config4_sampled(plic):
     """configs[3]: N = 2^28 cells (4.3 GB in, 1.1 GB out), half the normals snapped to an axis or a
     face diagonal, V0 ~ Beta(1/2, 1/2): properties on every cell, the oracle on every 1024th."""
