@@ -53,7 +53,8 @@ typedef struct CUstream_st *cudaStream_t;
 #define PLIC_FAST        0x100 /* approximate SFU roots/reciprocals/trig, branch-free a-priori
                                   case selection, two cells per packed fp32x2 instruction;
                                   without it: IEEE division and square root, CUDA libm
-                                  cbrt/asin/acos/sin/cos, branches in the paper's order */
+                                  cbrt/asin/acos/sin/cos, cases in the paper's order with the
+                                  expensive ones (1), (3), (4) evaluated in dense warps */
 
 /* ---- error codes (functions return 0 on success, never throw, never print) ---------------- */
 #define PLIC_OK               0
