@@ -404,6 +404,7 @@ def time_variants(plic, arrays, out, steps, warmup, stream, world, sampler, sms,
              "bytes_per_cell": BYTES_PER_CELL, "hbm_gbs_per_gpu": gbs, "hbm_frac": gbs / peak,
              "hbm_frac_nominal": gbs / NOMINAL_HBM_GBS, "sm_mhz": clk.get("sm_mhz")}
         e["roofline_frac"] = e["hbm_frac"]
+        e["_window"] = win
         issue_fields(e, counts.get(name), N, ms, sms, clk.get("sm_mhz"))
         if clk.get("sm_mhz"):
             # SURVEY.md 8d also asks for the issue fraction from the ALGORITHMIC counts: the thread-
@@ -527,10 +528,10 @@ def run_ours(args):
     head = args.method if args.method != "auto" else max(solve_names, key=lambda k: methods[k]["value"])
     H = methods[head]
     hm, hf = (head[:-5], True) if head.endswith("-fast") else (head, False)
-    # the headline once more for its clock window (the per-method windows are not kept)
-    _, head_win = time_launches(lambda: plic.plic_solve(dV, dx, dy, dz, out=out, method=hm, fast=hf),
-                                args.steps, args.warmup, stream)
-    windows[head] = head_win
+    # `clocks` is sampled inside the very window `value` was timed in (kept per variant by time_variants)
+    windows[head] = H.pop("_window")
+    for v in methods.values():
+        v.pop("_window", None)
 
     # ---- instruction rates of the pipes, measured here ("confirm with an FFMA-only and a
     # MUFU-only microbenchmark"): warp-instructions per sub-partition per clock at the sampled clock
@@ -650,6 +651,8 @@ def run_ours(args):
         del h4
         o4 = torch.empty_like(a4[0])
         r4 = time_variants(plic, a4, o4, args.steps, args.warmup, stream, world, sampler, sms, counts, peak)
+        for v in r4.values():
+            v.pop("_window", None)
         config4 = {"workload": "configs[3]: N=2^%d cells (%.1f GB in, %.1f GB out), seed 3, half the normals snapped to an "
                                "axis or a face diagonal, V0 ~ Beta(1/2,1/2)" % (args.config4_log2n, 16 * N4 / 1e9, 4 * N4 / 1e9),
                    "cells": N4, "generator_s": gen_s, "methods": r4}
@@ -769,7 +772,9 @@ def run_ours(args):
                        "l2": "inputs larger than L2 (1.07 GB read + 0.27 GB written per step vs 126 MB)",
                        "prewarm_ms": args.prewarm_ms, "launch": {"grid": plic.plic_launch_config(hm, N, hf)[0],
                                                                  "block": 256, "cells_per_thread": 4}},
-            "clocks": clocks,
+            "clocks": dict(clocks, window="the %d timed launches of the headline variant (`value`); under sustained load "
+                                          "this pool's boxes hold the SMs at 1.45-1.55 GHz (software power cap); `burst` "
+                                          "repeats the variant at full clock" % args.steps),
             "gpu_launches": H["launches"],
             "gpu_launches_all_timed_regions": total_launches,
             "e2e": {"value": N * world * e2e_steps / e2e_s / 1e9, "unit": UNIT,
