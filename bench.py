@@ -24,7 +24,9 @@ clock sampled in that method's timed window), issue slots = warp-instructions (n
 + packed fp32x2 warp-instructions (they hold the issue port for two clocks, see pipe_rates), both per
 cell from the committed table profiles/instruction_counts.txt; `bound` names the larger fraction;
 `issue_frac_algorithmic` is the same from SURVEY.md 8d's algorithmic operation counts (union of all case
-paths) against SMs x 128 FP32 lanes x clock.  "stream_ceiling" is the
+paths) against SMs x 128 FP32 lanes x clock; `per_launch` = median and best of 20 further launches, each
+between its own pair of events (2-3 % above ms_per_step: an event between two launches keeps the second
+from becoming resident while the first drains).  "stream_ceiling" is the
 same 4-read/1-write stream with no arithmetic (plic_solve with the blank method, d0 = V0 - 1/2);
 "pipe_rates" are the instruction rates of the FMA, SFU and ALU pipes measured in this run
 (plic_pipe_probe), from which the "alu" peak of the compute-bound legs is derived.
@@ -382,6 +384,21 @@ def pcie_link(sampler):
         return None
 
 
+def per_launch_stats(fn, n, stream):
+    """Median and best of n single launches, each bracketed by its own pair of CUDA events (SURVEY.md
+    8d, "Timing": median and best).  Separate from the timed region of `value`: an event between two
+    launches keeps the second from becoming resident while the first drains."""
+    import torch
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(n + 1)]
+    ev[0].record(stream)
+    for i in range(n):
+        fn()
+        ev[i + 1].record(stream)
+    torch.cuda.synchronize()
+    t = sorted(ev[i].elapsed_time(ev[i + 1]) for i in range(n))
+    return {"n": n, "median_ms": t[n // 2], "best_ms": t[0]}
+
+
 VARIANTS = [(m, f) for f in (True, False) for m in ("analytic", "sz", "newton", "nested")]
 # SURVEY.md 8d, "Algorithmic work per cell": FP32 + SFU operations of the union of all case paths
 ALGORITHMIC_INST = {"analytic": 95 + 7, "sz": 95 + 7, "newton": 105 + 8, "nested": 190 + 3}
@@ -404,6 +421,7 @@ def time_variants(plic, arrays, out, steps, warmup, stream, world, sampler, sms,
              "bytes_per_cell": BYTES_PER_CELL, "hbm_gbs_per_gpu": gbs, "hbm_frac": gbs / peak,
              "hbm_frac_nominal": gbs / NOMINAL_HBM_GBS, "sm_mhz": clk.get("sm_mhz")}
         e["roofline_frac"] = e["hbm_frac"]
+        e["per_launch"] = per_launch_stats(lambda: plic.plic_solve(*arrays, out=out, method=m, fast=f), 20, stream)
         e["_window"] = win
         issue_fields(e, counts.get(name), N, ms, sms, clk.get("sm_mhz"))
         if clk.get("sm_mhz"):
