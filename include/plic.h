@@ -64,6 +64,8 @@ typedef struct CUstream_st *cudaStream_t;
 #define PLIC_ERR_METHOD      -3 /* unknown method id */
 #define PLIC_ERR_LAUNCH      -4 /* the CUDA runtime reported an error (launch, copy, alloc) */
 #define PLIC_ERR_ALIGN       -5 /* a pointer is not aligned to its element size (4 bytes for fp32) */
+#define PLIC_ERR_CAPACITY    -6 /* plic_curvature_static only: the lattice has more interior cells than
+                                   PLIC_CURVATURE_STATIC_MAX_POINTS; nothing was enqueued */
 
 /*
  * plic_solve -- d0[i] = d0(V0[i], n[i]) for i in [0, N)            (eq. (1))
@@ -226,6 +228,49 @@ int plic_sphere_volume(const float *d0, float *V0, int64_t N, cudaStream_t strea
  */
 int plic_curvature(const float *phi, float *kappa, int nx, int ny, int nz, int32_t *work,
                    int64_t work_entries, cudaStream_t stream);
+
+/*
+ * plic_curvature_static -- plic_curvature without a `work` argument, for callers that cannot allocate
+ * device memory at the point where they need curvature.
+ *
+ * Who that is: a flow solver that gave all of the GPU's memory to its lattices at start-up and has
+ * nothing left to ask for (a cudaMalloc deep into a run fails, or starts failing after the next lattice
+ * resize); an application whose device memory is managed by its own pool or accounting layer, which a
+ * library must not bypass; a time-step loop that cannot afford cudaMalloc / cudaFree, both of which
+ * synchronise the whole device and stall every stream.  plic_curvature asks such a caller for scratch
+ * it cannot produce.  Here the interface list is a fixed array inside the library instead: it is part
+ * of the library's device image, so a GPU holds it (16 MiB) from the moment the library's device code
+ * is loaded onto it until the process exits, whether or not this function is ever called again.  The
+ * call itself allocates and frees nothing, directly or through any library routine.
+ *
+ *   phi, kappa, nx, ny, nz, stream   exactly as plic_curvature; the caller still owns input and output.
+ *
+ * Limit: the list holds PLIC_CURVATURE_STATIC_MAX_POINTS cell indices.  Only cells with a full 3^3
+ * neighbourhood are listed, so a lattice is accepted when (nx-2)(ny-2)(nz-2) does not exceed that
+ * number -- e.g. up to 163^3, or 1026 x 1026 x 6 -- and the result is then always complete (bitwise the
+ * kappa of plic_curvature with a large enough `work`).  A larger lattice is refused with
+ * PLIC_ERR_CAPACITY before anything is enqueued, even if it happens to contain few interface cells:
+ * use plic_curvature with caller-owned scratch for those.
+ *
+ * First call on each device: the function looks up the array's device address (cudaGetSymbolAddress,
+ * with that device current; the CUDA runtime may load the library's device code onto the GPU at this
+ * moment) and remembers it.  Make that first call during start-up, outside any stream capture and
+ * before the phase in which allocation is impossible; a call with an empty lattice
+ * (nx = 0, phi = kappa = NULL) does the look-up and nothing else.  If the look-up fails the call returns
+ * PLIC_ERR_LAUNCH and the next call tries again.
+ *
+ * One list per GPU, shared by every call: the list still holds the previous call's entries when the
+ * next call starts (the call's first kernel clears the counter, which is all that has to start at
+ * zero).  Two calls on the same GPU whose kernels can overlap -- different streams without an event
+ * between them, or several host threads -- race on the list and give wrong kappa.  Calls on one stream,
+ * or ordered by events, are safe; so are calls on different GPUs.  The interface count and list are not
+ * returned; a caller that needs them uses plic_curvature.
+ *
+ * Returns PLIC_OK, PLIC_ERR_SIZE (negative extents, >= 2^31 cells), PLIC_ERR_CAPACITY, PLIC_ERR_NULL,
+ * PLIC_ERR_ALIGN or PLIC_ERR_LAUNCH.
+ */
+#define PLIC_CURVATURE_STATIC_MAX_POINTS 4194303 /* 2^22 - 1: with the counter, 16 MiB of int32 */
+int plic_curvature_static(const float *phi, float *kappa, int nx, int ny, int nz, cudaStream_t stream);
 
 /*
  * plic_solve_host / plic_volume_host -- the same maps for HOST arrays (pageable or pinned;

@@ -18,6 +18,9 @@ shared library is missing it is built with nvcc, and if that fails the import ra
                                             the plane-sphere intersection of sect. 3
     plic_curvature(phi, out=None, work=None) -> kappa
                                             curvature from a lattice of fill levels, sect. 4
+    plic_curvature_static(phi, out=None) -> kappa
+                                            the same without scratch from the caller (built-in list,
+                                            lattices up to CURVATURE_STATIC_MAX_POINTS interior cells)
 """
 from __future__ import annotations
 
@@ -29,6 +32,7 @@ from . import build as _build
 __all__ = ["METHODS", "FAST", "BLANK", "KAWANO", "method_id", "plic_solve", "plic_volume",
            "plic_solve_h", "plic_volume_h", "plic_solve_f64",
            "plic_roundtrip_error", "plic_sphere_solve", "plic_sphere_volume", "plic_curvature",
+           "plic_curvature_static", "CURVATURE_STATIC_MAX_POINTS",
            "plic_solve_host",
            "plic_volume_host", "plic_host_release", "plic_method_name", "plic_error_string",
            "plic_version", "plic_launch_config", "plic_pipe_probe", "PROBES", "plic_launch_count", "PlicError", "lib",
@@ -38,6 +42,7 @@ METHODS = {"analytic": 0, "sz": 1, "newton": 2, "nested": 3}
 KAWANO = 4              # Listing 3 (Kawano's SZ translation), precise only; see include/plic.h
 FAST = 0x100
 BLANK = 0x40            # plic_roundtrip_error only: the blank run of eq. (33)
+CURVATURE_STATIC_MAX_POINTS = (1 << 22) - 1     # PLIC_CURVATURE_STATIC_MAX_POINTS of include/plic.h
 LIB_PATH = _build.LIB
 
 
@@ -73,6 +78,8 @@ def _load() -> ctypes.CDLL:
     lib_.plic_curvature.argtypes = [fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, fp, i64,
                                     ctypes.c_void_p]
     lib_.plic_curvature.restype = ctypes.c_int
+    lib_.plic_curvature_static.argtypes = [fp, fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_void_p]
+    lib_.plic_curvature_static.restype = ctypes.c_int
     lib_.plic_solve_host.argtypes = [fp, fp, fp, fp, fp, i64, ctypes.c_int]
     lib_.plic_solve_host.restype = ctypes.c_int
     lib_.plic_volume_host.argtypes = [fp, fp, fp, fp, fp, i64]
@@ -328,6 +335,36 @@ def plic_curvature(phi, out=None, work=None, stream=None):
                                 work.numel(), _stream_handle(stream, phi.device))
     if rc != 0:
         raise PlicError(rc, "plic_curvature")
+    return out
+
+
+def plic_curvature_static(phi, out=None, stream=None):
+    """plic_curvature for callers that cannot allocate device memory where they need curvature (a solver
+    whose lattices already fill the GPU, an application with its own device-memory pool, a time-step
+    loop that must not hit cudaMalloc's device-wide synchronisation): the interface list is a fixed
+    16 MiB array inside libplic instead of a `work` tensor.  Pass `out` (e.g. a buffer of the solver)
+    and the call allocates nothing at all; with out=None only the result tensor comes from torch.
+
+    Accepts lattices with at most CURVATURE_STATIC_MAX_POINTS cells off the border ((nx-2)(ny-2)(nz-2),
+    e.g. 163^3); larger ones raise PlicError (code -6) before any GPU work -- use plic_curvature there.
+    The first call on a device looks up the array's address: make it at start-up, outside stream
+    capture.  All calls on one GPU share the list, so calls that may overlap on the GPU (two streams
+    with no event between them) race; calls on one stream are fine.  kappa is bitwise that of
+    plic_curvature.  Returns `out`."""
+    import torch
+    if not (phi.is_cuda and phi.dtype == torch.float32 and phi.dim() == 3 and phi.is_contiguous()):
+        raise ValueError("phi must be a contiguous 3-D float32 CUDA tensor [nz, ny, nx]")
+    if out is None:
+        out = torch.empty_like(phi)
+    elif not (out.is_cuda and out.dtype == torch.float32 and out.is_contiguous()
+              and out.shape == phi.shape and out.device == phi.device):
+        raise ValueError("out must be a contiguous float32 CUDA tensor of phi's shape")
+    nz, ny, nx = phi.shape
+    with torch.cuda.device(phi.device):
+        rc = lib.plic_curvature_static(phi.data_ptr(), out.data_ptr(), nx, ny, nz,
+                                       _stream_handle(stream, phi.device))
+    if rc != 0:
+        raise PlicError(rc, "plic_curvature_static")
     return out
 
 

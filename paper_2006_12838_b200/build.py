@@ -21,7 +21,7 @@ SOURCES = [os.path.join(CSRC, "plic_kernels.cu")]
 DEPENDS = SOURCES + [os.path.join(CSRC, "plic_methods.cuh"), os.path.join(CSRC, "plic_math.cuh"),
                      os.path.join(CSRC, "plic_packed.cuh"), os.path.join(CSRC, "plic_curvature.cuh"),
                      os.path.join(CSRC, "plic_probe.cuh"), os.path.join(CSRC, "plic_storage.cuh"),
-                     os.path.join(CSRC, "plic_f64.cuh"),
+                     os.path.join(CSRC, "plic_f64.cuh"), os.path.join(CSRC, "plic_curvature_static.cuh"),
                      os.path.join(ROOT, "include", "plic.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

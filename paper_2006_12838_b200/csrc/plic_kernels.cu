@@ -884,6 +884,9 @@ const char *plic_error_string(int code) {
         case PLIC_ERR_METHOD: return "unknown method id";
         case PLIC_ERR_LAUNCH: return "CUDA runtime error";
         case PLIC_ERR_ALIGN: return "pointer not aligned to its element size";
+        case PLIC_ERR_CAPACITY:
+            return "lattice has more interior cells than plic_curvature_static's built-in list holds "
+                   "(PLIC_CURVATURE_STATIC_MAX_POINTS); use plic_curvature with your own work array";
         default: return "unknown error code";
     }
 }
@@ -957,3 +960,5 @@ int plic_launch_config(int method, int64_t N, int *grid, int *block, int *cells_
 int64_t plic_launch_count(void) { return plic::g_launches.load(std::memory_order_relaxed); }
 
 }  // extern "C"
+
+#include "plic_curvature_static.cuh"   // plic_curvature_static: the curvature call with a built-in interface list
