@@ -54,8 +54,10 @@ cells / max-over-ranks time ("scaling": "weak").  Under torchrun the ranks come 
 environment; a plain `python bench.py --gpus N` (N > 1) re-launches itself under
 torch.distributed.run with N ranks on 127.0.0.1.
 
-The last key, "summary", repeats the per-variant results in compact form (drivers that keep only
-the tail of the line still see them).
+Output: stdout carries ONE line, the compact contract line (compact_line: under 8000 bytes -- the
+contract keys, `roofline`, `cpu_baseline`, `e2e`, `clocks` and a per-variant `summary`).  The full
+object with every variant of every leg ("methods", "storage", "pipe_rates", "paper_benchmark",
+"divergence", "config4"; 30+ KB) is written to --detail-out (default bench_detail.json, git-ignored).
 
 --impl reference times the fp64 CPU oracle (oracle/), as it stands, on the host cores.
 """
@@ -203,6 +205,7 @@ class ClockSampler:
         reasons = [name for bit, name in self.REASONS.items() if mask & bit]
         pw = [s[3] for s in ins if s[3] is not None]
         return {"sm_mhz": clocks[len(clocks) // 2], "sm_min_mhz": clocks[0], "sm_max_mhz": self.sm_max,
+                "sm_mean_mhz": round(sum(clocks) / len(clocks), 1), "sm_top_mhz": clocks[-1],
                 "reasons": reasons, "samples": len(ins), "power_w_max": max(pw) if pw else None,
                 "note": note}
 
@@ -404,16 +407,19 @@ VARIANTS = [(m, f) for f in (True, False) for m in ("analytic", "sz", "newton", 
 ALGORITHMIC_INST = {"analytic": 95 + 7, "sz": 95 + 7, "newton": 105 + 8, "nested": 190 + 3}
 
 
-def time_variants(plic, arrays, out, steps, warmup, stream, world, sampler, sms, counts, peak):
+def time_variants(plic, arrays, out, steps, warmup, stream, world, sampler, sms, counts, peak, workload="configs[1]"):
     """Times the eight plic_solve variants on `arrays`; one dict per variant with both HBM fractions,
-    the issue fraction at the clock sampled in its own window, and the binding roofline."""
+    the issue fraction at the clock sampled in its own window, and the binding roofline.  `workload`
+    names the arrays (configs[k]): executed-instruction counts of the data-dependent kernels are used
+    only when profiles/instruction_counts.txt was captured on that workload."""
     N = arrays[0].numel()
     res = {}
     for m, f in VARIANTS:
         name = plic.plic_method_name(plic.method_id(m, f))
         c0 = plic.plic_launch_count()
         ms, win = time_launches(lambda: plic.plic_solve(*arrays, out=out, method=m, fast=f), steps, warmup, stream)
-        launches = (plic.plic_launch_count() - c0) - warmup
+        # kernels per timed step x steps (a call with a misaligned head or a ragged tail is two launches)
+        launches = (plic.plic_launch_count() - c0) * steps // (steps + warmup)
         ms = max_over_ranks(ms) / steps
         clk = sampler.summary([win])
         gbs = BYTES_PER_CELL * N / (ms * 1e-3) / 1e9
@@ -423,7 +429,7 @@ def time_variants(plic, arrays, out, steps, warmup, stream, world, sampler, sms,
         e["roofline_frac"] = e["hbm_frac"]
         e["per_launch"] = per_launch_stats(lambda: plic.plic_solve(*arrays, out=out, method=m, fast=f), 20, stream)
         e["_window"] = win
-        issue_fields(e, counts.get(name), N, ms, sms, clk.get("sm_mhz"))
+        issue_fields(e, counts_row(counts, name, workload), N, ms, sms, clk)
         if clk.get("sm_mhz"):
             # SURVEY.md 8d also asks for the issue fraction from the ALGORITHMIC counts: the thread-
             # instructions per cell a mixed warp has to issue for the method's formulas (union of all
@@ -434,22 +440,51 @@ def time_variants(plic, arrays, out, steps, warmup, stream, world, sampler, sms,
     return res
 
 
-def issue_fields(e, row, N, ms, sms, mhz):
+DATA_DEPENDENT_KERNELS = ("map_compact",)      # per-tile compaction of the heavy cases, bisection to convergence
+
+
+def counts_row(counts, name, workload):
+    """Row of profiles/instruction_counts.txt for kernel `name` timed on `workload`, or None when the row
+    cannot describe that run: the table carries the workload it was captured on ('#@ workload'), and the
+    executed count of a data-dependent kernel (DATA_DEPENDENT_KERNELS) on another workload is a different
+    number.  Branch-free kernels execute the same instructions on any input, so their row always applies."""
+    row = counts.get(name)
+    if row is None:
+        return None
+    captured_on = counts.get("@workload", ["configs[1]"])[0]
+    kernel = row[3] if len(row) > 3 else ""
+    if workload != captured_on and kernel.startswith(DATA_DEPENDENT_KERNELS):
+        return None
+    return row
+
+
+def issue_fields(e, row, N, ms, sms, clk):
     """Issue roofline of one timed kernel from its row of profiles/instruction_counts.txt.  A packed
     fp32x2 instruction (FFMA2/FMUL2/FADD2) holds the issue port of its SM sub-partition for two
     clocks (pipe_rates: ffma2 alone 0.50 per clock, ffma2 + lop3 0.66 = 3 clocks per pair), every
     other instruction for one, so issue slots per cell = warp-instructions + packed warp-instructions;
-    issue_frac = slots per cell x cells/s / (SMs x 4 sub-partitions x the SM clock sampled in this
-    kernel's timed window)."""
+    issue_frac = slots per cell x cells/s / (SMs x 4 sub-partitions x the MEAN SM clock of the NVML
+    samples inside this kernel's timed window).  No row (none captured, or captured on another workload
+    for a data-dependent kernel): issue_frac is None.  A fraction above 1 cannot be a measurement -- the
+    counts or the clock do not belong to this run -- so it is flagged (`issue_model_error`) and does not
+    pick `bound`."""
+    clk = clk if isinstance(clk, dict) else {"sm_mhz": clk, "sm_mean_mhz": clk}
+    mhz = clk.get("sm_mean_mhz") or clk.get("sm_mhz")
     if row is None or not mhz:
+        e["issue_frac"] = None
         return
     wipc, packed = float(row[0]), float(row[2])
     e["warp_inst_per_cell"] = wipc
     e["lanes_per_inst"] = float(row[1])
     e["packed_warp_inst_per_cell"] = packed
     e["issue_slots_per_cell"] = wipc + packed
+    e["issue_clock_mhz"] = mhz
     e["issue_frac"] = (wipc + packed) * N / (ms * 1e-3) / (sms * 4 * mhz * 1e6)
-    e["bound"] = "issue" if e["issue_frac"] > e["hbm_frac"] else "hbm"
+    if e["issue_frac"] > 1.0:
+        e["issue_model_error"] = True
+        e["bound"] = None
+    else:
+        e["bound"] = "issue" if e["issue_frac"] > e["hbm_frac"] else "hbm"
 
 
 def run_ours(args):
@@ -502,7 +537,7 @@ def run_ours(args):
         e = {"value": N * world / (ms * 1e-3) / 1e9, "ms_per_step": ms, "launches": args.steps,
              "bytes_per_cell": bytes_per_cell, "hbm_gbs_per_gpu": gbs, "hbm_frac": gbs / peak,
              "hbm_frac_nominal": gbs / NOMINAL_HBM_GBS, "roofline_frac": gbs / peak, "sm_mhz": clk.get("sm_mhz")}
-        issue_fields(e, counts.get(name), N, ms, sms, clk.get("sm_mhz"))
+        issue_fields(e, counts.get(name), N, ms, sms, clk)
         return e
 
     # the 4-read / 1-write stream with no arithmetic, in the same sustained regime
@@ -649,7 +684,8 @@ def run_ours(args):
         r = {}
         for lay in ("interleaved", "contiguous"):
             a = [torch.from_numpy(t if lay == "interleaved" else t[order]).cuda() for t in (sV, sx, sy, sz)]
-            r[lay] = time_variants(plic, a, out, args.steps, args.warmup, stream, world, sampler, sms, counts, peak)
+            r[lay] = time_variants(plic, a, out, args.steps, args.warmup, stream, world, sampler, sms, counts, peak,
+                                   workload="configs[2]")
             del a
         for name in solve_names:
             i_, c_ = r["interleaved"][name], r["contiguous"][name]
@@ -668,7 +704,8 @@ def run_ours(args):
         a4 = [torch.from_numpy(t).cuda() for t in h4]
         del h4
         o4 = torch.empty_like(a4[0])
-        r4 = time_variants(plic, a4, o4, args.steps, args.warmup, stream, world, sampler, sms, counts, peak)
+        r4 = time_variants(plic, a4, o4, args.steps, args.warmup, stream, world, sampler, sms, counts, peak,
+                           workload="configs[3]")
         for v in r4.values():
             v.pop("_window", None)
         config4 = {"workload": "configs[3]: N=2^%d cells (%.1f GB in, %.1f GB out), seed 3, half the normals snapped to an "
@@ -852,12 +889,65 @@ def run_ours(args):
             "curvature_ms": None if curv is None else round(curv["ms_per_call"], 4),
             "storage_ms": None if storage is None else {k: round(v["ms_per_step"], 4) for k, v in storage.items()},
         }
-        print(json.dumps(line), flush=True)
+        detail_path = write_detail(line, args.detail_out)
+        print(json.dumps(compact_line(line, detail_path)), flush=True)     # the ONLY stdout line
     if world > 1:
         import torch.distributed as dist
         dist.barrier()
         dist.destroy_process_group()
     return 0
+
+
+# ---- what goes to stdout: one contract line a driver can parse from a bounded tail ----------------
+LINE_LIMIT = 8000        # bytes; the full object (30+ KB: every variant of every leg) goes to --detail-out
+DETAIL_KEYS = ("methods", "storage", "pipe_rates", "paper_benchmark", "divergence", "config4")
+_DROP_IF_LONG = ("stream_ceiling", "burst", "curvature", "cpu_baseline_1core")   # in this order
+
+
+def _round_floats(x, digits=6):
+    if isinstance(x, float):
+        return float("%.*g" % (digits, x)) if x == x and abs(x) != float("inf") else None
+    if isinstance(x, dict):
+        return {k: _round_floats(v, digits) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_round_floats(v, digits) for v in x]
+    return x
+
+
+def compact_line(line, detail_path=None):
+    """The contract line printed last on stdout: every key the bench contract names (metric, value, unit,
+    n_gpus, steps, warmup, ms_per_step, higher_is_better, scaling, vs_baseline, dtype, data, config, clocks,
+    gpu_launches, e2e, roofline, cpu_baseline) plus the per-variant `summary`, without the per-leg detail
+    objects (DETAIL_KEYS), floats at 6 significant digits, and guaranteed shorter than LINE_LIMIT bytes so
+    that a driver which keeps only the tail of stdout still holds the whole line."""
+    out = {k: v for k, v in line.items() if k not in DETAIL_KEYS}
+    out = _round_floats(out)
+    out["detail"] = {"file": detail_path, "keys": [k for k in DETAIL_KEYS if k in line]}
+    for k in (None,) + _DROP_IF_LONG:
+        if k is not None:
+            out.pop(k, None)
+        if len(json.dumps(out)) < LINE_LIMIT:
+            return out
+    if isinstance(out.get("summary"), dict):
+        out["summary"].pop("storage_ms", None)
+    if len(json.dumps(out)) >= LINE_LIMIT:
+        out.pop("summary", None)
+    return out
+
+
+def write_detail(line, path):
+    """The full result object as indented JSON in `path` (None or "" skips it); returns the path written."""
+    if not path:
+        return None
+    try:
+        os.makedirs(os.path.dirname(os.path.abspath(path)), exist_ok=True)
+        with open(path, "w") as f:
+            json.dump(line, f, indent=1)
+            f.write("\n")
+        return path
+    except OSError as e:
+        sys.stderr.write("bench.py: could not write %s (%s)\n" % (path, e))
+        return None
 
 
 def run_plumbing_only(args):
@@ -919,6 +1009,9 @@ def main(argv=None):
     ap.add_argument("--config4-log2n", type=int, default=28)
     ap.add_argument("--no-probes", action="store_true", help="skip the instruction-rate probes")
     ap.add_argument("--no-storage", action="store_true", help="skip the fp16-storage / fp64 variants")
+    ap.add_argument("--detail-out", default=os.path.join(ROOT, "bench_detail.json"),
+                    help="file for the full result object (every variant of every leg); stdout carries only "
+                         "the compact contract line.  '' skips the file")
     ap.add_argument("--plumbing-only", action="store_true",
                     help="exercise the multi-rank launch and reductions on CPU (gloo); no GPU work, no metric")
     ap.add_argument("--paper-log2n", type=int, default=24,

@@ -35,6 +35,25 @@
 #pragma once
 #include "plic_packed.cuh"
 
+// ---- tuning switches of the point pass (curvature_point, curv_cells) --------------------------------
+// Defined here, ahead of every use: an `#if` on a macro that is only defined further down silently takes
+// the 0 branch (this is how round 2 shipped KEEP = 0 while the text said 1).
+#ifndef PLIC_CURV_KEEP
+#define PLIC_CURV_KEEP 1     // keep the 26 fill levels in registers between step 1 and step 3 (0: read them again, L1 hits)
+#endif
+#ifndef PLIC_CURV_LANES
+#define PLIC_CURV_LANES 1
+#endif
+#ifndef PLIC_CURV_BLOCK
+#define PLIC_CURV_BLOCK 64
+#endif
+#ifndef PLIC_CURV_MINBLOCKS
+#define PLIC_CURV_MINBLOCKS 7
+#endif
+#if PLIC_CURV_KEEP != 0 && PLIC_CURV_KEEP != 1
+#error "PLIC_CURV_KEEP must be 0 or 1"
+#endif
+
 namespace plic {
 
 
@@ -217,7 +236,8 @@ __device__ __forceinline__ float curvature_point(const float *__restrict__ phi, 
     float keep_p[SLOTS], keep_m[SLOTS];
 #endif
     // step 1: eq. (54), weights eq. (55): 4, 2, 1 for |e|_1 = 1, 2, 3; the pair contributes w e (phi+ - phi-).
-    // The fill levels are not kept: step 3 reads them again (L1 hits), which frees ~35 registers.
+    // PLIC_CURV_KEEP = 1: the 26 fill levels stay in registers for step 3; 0: step 3 reads them again
+    // (L1 hits), which frees ~35 registers.
 #pragma unroll
     for (int s = 0; s < SLOTS; ++s) {
         const int k = sub + LANES * s;
@@ -342,18 +362,6 @@ __device__ __forceinline__ float curvature_point(const float *__restrict__ phi, 
 }
 
 // ---- curv_cells: kPointLanes lanes per entry of the caller's list ------------------------------------
-#ifndef PLIC_CURV_KEEP
-#define PLIC_CURV_KEEP 1     // keep the 26 fill levels in registers between step 1 and step 3 (0: read them again, L1 hits)
-#endif
-#ifndef PLIC_CURV_LANES
-#define PLIC_CURV_LANES 1
-#endif
-#ifndef PLIC_CURV_BLOCK
-#define PLIC_CURV_BLOCK 64
-#endif
-#ifndef PLIC_CURV_MINBLOCKS
-#define PLIC_CURV_MINBLOCKS 7
-#endif
 constexpr int kPointLanes = PLIC_CURV_LANES;
 constexpr int kCurvBlock = PLIC_CURV_BLOCK;    // threads per block
 
