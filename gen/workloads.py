@@ -3,8 +3,8 @@
 Nothing here evaluates the PLIC forward or inverse map, classifies an
 intersection case, or sorts a normal: the generators only draw normals and
 volumes with the distributions BASELINE.json's configs name.  (The
-case-stratified config 3 needs the oracle's forward map and therefore lives in
-tests/stratified.py, not here.)
+case-stratified configs[2] needs the oracle's forward map and classifier and
+therefore lives in oracle/stratified.c / oracle/stratified.py, not here.)
 """
 from __future__ import annotations
 

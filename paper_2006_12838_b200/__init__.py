@@ -41,7 +41,7 @@ __all__ = ["METHODS", "FAST", "BLANK", "KAWANO", "method_id", "plic_solve", "pli
 METHODS = {"analytic": 0, "sz": 1, "newton": 2, "nested": 3}
 KAWANO = 4              # Listing 3 (Kawano's SZ translation), precise only; see include/plic.h
 FAST = 0x100
-BLANK = 0x40            # plic_roundtrip_error only: the blank run of eq. (33)
+BLANK = 0x40            # the blank run of eq. (33): d0 = V0 - 1/2 (plic_roundtrip_error, plic_solve, plic_solve_h)
 CURVATURE_STATIC_MAX_POINTS = (1 << 22) - 1     # PLIC_CURVATURE_STATIC_MAX_POINTS of include/plic.h
 LIB_PATH = _build.LIB
 

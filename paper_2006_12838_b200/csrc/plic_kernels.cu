@@ -294,8 +294,10 @@ map_compact(const float4 *s, const float4 *__restrict__ nx, const float4 *__rest
     grid_dependency_wait();
     const int64_t i = (int64_t)blockIdx.x * kBlock + tid;
     const bool live = i < n4;
-    // threads past the end carry the zero normal: case (5), nothing queued
-    float4 v = make_float4(0.f, 0.f, 0.f, 0.f), a = v, b = v, c = v;
+    // threads past the end carry n = (0, 0, 1), V0 = 0: case (5) in every method (n1 + n2 = 0 <= 2 V n3 = 0),
+    // nothing queued.  (The zero normal would not do: SZ divides by S = 0 and its NaN fails every case
+    // test, which queues the dead slots as heavy cells.)
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f), a = v, b = v, c = make_float4(1.f, 1.f, 1.f, 1.f);
     if (live) {
         v = ld_stream_rw(s + i);
         a = ld_stream(nx + i);

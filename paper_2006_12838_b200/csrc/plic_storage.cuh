@@ -216,7 +216,10 @@ map_compact_io(const void *s, const void *nx, const void *ny, const void *nz, vo
     const bool live = i < nvec;
     real V0[P], X[P], Y[P], Z[P];
 #pragma unroll
-    for (int k = 0; k < P; ++k) V0[k] = X[k] = Y[k] = Z[k] = (real)0;      // past the end: case (5), nothing queued
+    for (int k = 0; k < P; ++k) {                    // past the end: n = (0, 0, 1), V0 = 0 is case (5) in every
+        V0[k] = X[k] = Y[k] = (real)0;               // method, nothing queued (the zero normal would make SZ's
+        Z[k] = (real)1;                              // 1/S a NaN and queue the dead slots as heavy cells)
+    }
     if (live) {
         IO::load(s, i, true, V0);
         IO::load(nx, i, false, X);
