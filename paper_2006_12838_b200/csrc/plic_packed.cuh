@@ -324,10 +324,16 @@ struct PairSolver<NEWTON> {
 };
 
 // ---------------------------------------------------------------------------------------
-// method 3, PLIC_FAST: nested intervals (sect. 2.5) on a pair: 20 fixed halvings of the
-// bracket [lo, hi] of the depressed cubic F for (3)/(4) (|err| <= 3.3e-7; the precise kernel
-// halves until the fp32 midpoint stops moving); closed forms for (1), (2), (5).  F is
-// decreasing on the bracket, F(lo) >= 0 >= F(hi).
+// method 3, PLIC_FAST: nested intervals (sect. 2.5) on a pair: kNestedFastHalvings = 16 fixed
+// halvings of the bracket [lo, hi] of the depressed cubic F for (3)/(4); closed forms for (1),
+// (2), (5).  F is decreasing on the bracket, F(lo) >= 0 >= F(hi).
+// Accuracy is bought per halving: after N halvings the centre is within w 2^-(N+1) of the root,
+// w = hi - lo <= n1 <= 0.577, i.e. |err| <= 4.4e-6 for N = 16 -- 4.5 times inside the 2e-5 bar, and
+// the forward-volume residual (dV/dd0 = area of the cut <= sqrt 2) <= 6.3e-6.  Rounds 1-2 ran
+// N = 20 (|err| <= 2.9e-7 observed) at 20 x 8 issue slots per pair, which left the kernel at half
+// its HBM roofline; the precise kernel (no PLIC_FAST) still halves until the fp32 midpoint stops
+// moving, as the paper's listing does.  -DPLIC_NESTED_FAST_HALVINGS=20
+// rebuilds the old trade.
 //
 // The halving runs in the scaled variable y = tau / (hi - lo), in which the bracket has unit
 // width, and carries the interval's CENTRE c instead of its lower end:
@@ -358,6 +364,13 @@ __device__ __forceinline__ float signed_step(float G, unsigned mask) {
     asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(r) : "r"(__float_as_uint(G)), "r"(mask), "n"(STEP_BITS));
     return __uint_as_float(r);
 }
+
+#ifndef PLIC_NESTED_FAST_HALVINGS
+#define PLIC_NESTED_FAST_HALVINGS 16
+#endif
+constexpr int kNestedFastHalvings = PLIC_NESTED_FAST_HALVINGS;
+static_assert(kNestedFastHalvings >= 14 && kNestedFastHalvings <= 22,
+              "14 halvings are 1.8e-5 (no margin to the 2e-5 bar), beyond 22 the step falls below an fp32 ulp of c");
 
 template <int K, int N>
 struct NestedSteps {
@@ -403,7 +416,7 @@ struct PairSolver<NESTED> {
         const F2 nP = mul2(np, iw2);                                            // -p / w^2
         const F2 nR = mul2(mul2(nr, iw), iw2);                                  // -r / w^3
         F2 c = fma2(lo, iw, f2(0.5f));
-        NestedSteps<0, 20>::run(c, nP, nR, sign_mask_register());
+        NestedSteps<0, kNestedFastHalvings>::run(c, nP, nR, sign_mask_register());
         const F2 d34 = max2(fma2(c, w, sel2(c4, in.hS, n12)), n2);              // floor; drops NaN
         d = sel2(gt2(t1, mul2(n2, sub2(n2, n1))), d34, d);
         return pair_residual(in, d, W, h);

@@ -95,6 +95,13 @@ def test_config1_observed_error_regression(plic, config1, method, fast):
     V0, nx, ny, nz, ref = config1
     got = plic.plic_solve(*dev(V0, nx, ny, nz), method=method, fast=fast).cpu().numpy()
     err = np.abs(got.astype(np.float64) - ref)
+    if method == "nested" and fast:
+        # round 3: 16 fixed halvings instead of 20 (14 halvings give
+        # 1.2e-5, 20 give 2.9e-7).  The centre after 16 halvings is within w 2^-17 <= 0.577 * 2^-17 =
+        # 4.4e-6 of the root (w = bracket width <= n1), plus fp32 rounding; the parity bar stays 2e-5.
+        assert err.max() <= 4.8e-6, err.max()
+        assert err.mean() <= 1.0e-6, err.mean()
+        return
     assert err.max() <= (1.5e-6 if fast else 6e-7), err.max()
     assert err.mean() <= (1.5e-7 if fast else 6e-8), err.mean()
 
