@@ -38,7 +38,8 @@ rejection sampling on the oracle's classifier, V0 by the oracle's forward map), 
 "config4" = configs[3], 2^28 cells, half the normals snapped to an axis or face diagonal,
 V0 ~ Beta(1/2,1/2) (gen.snapped_beta), all 8 variants; "curvature" = plic_curvature on configs[4]
 (256^3 lattice, sphere R = 60), rotating over three copies of the lattice so that no call finds its
-input in L2, with the curvature oracle beside it.  "paper_benchmark" is the paper's own benchmark
+input in L2, with the curvature oracle beside it, and ("large") the same call on the 400 x 400 x 340
+lattice of the paper's raindrop run holding a sphere of radius 120.  "paper_benchmark" is the paper's own benchmark
 shape (sect. 2.6, Table 3) through plic_roundtrip_error: 2^k normals x L = 256 volumes in series per
 thread, blank run (eq. 33) subtracted, ps per PLIC evaluation and E_avg (eq. 32) per method --
 compute bound, for comparison with the paper's Titan Xp column (context, not the target).
@@ -759,6 +760,36 @@ def run_ours(args):
                                     "cores": _o.max_threads(), "kind": "oracle",
                                     "sample": "the whole 256^3 lattice once (%.1f s)" % dt}
         del phis, kaps, work5, host_phi
+        # ---- the same call at the lattice size the paper's raindrop run uses (400 x 400 x 340 =
+        # 54.4 M lattice points): the launch chain and the dependent point pass are a fixed ~12 us, so the
+        # larger lattice separates them from the stream (435 MB read + written per call)
+        if not args.no_curvature_large:
+            RL = 120.0
+            t0 = time.perf_counter()
+            big = np.ascontiguousarray(gen.sphere_fill_lattice(400, RL, (200.3, 199.7, 170.1), 8)[:340])
+            gen_s = time.perf_counter() - t0
+            phis = [torch.from_numpy(big).cuda() for _ in range(3)]
+            kaps = [torch.empty_like(p_) for p_ in phis]
+            workL = torch.empty(1 + phis[0].numel(), dtype=torch.int32, device="cuda")
+            turn[0] = 0
+
+            def curv_call_large():
+                j = turn[0] % 3
+                turn[0] += 1
+                plic.plic_curvature(phis[j], out=kaps[j], work=workL)
+            ms, _ = time_launches(curv_call_large, args.steps, args.warmup, stream)
+            ms = max_over_ranks(ms) / args.steps
+            ncell = phis[0].numel()
+            kk = -kaps[0][kaps[0] != 0].double() * RL
+            curv["large"] = {"workload": "400 x 400 x 340 lattice (PAPER.md:422), sphere R=120 at (200.3,199.7,170.1), same "
+                                         "generator and sub-sampling as configs[4]; three copies in turn (L2-cold)",
+                             "lattice_cells": ncell, "ms_per_call": ms, "interface_points": int(workL[0].item()),
+                             "lattice_gcells_per_s": ncell / (ms * 1e-3) / 1e9,
+                             "hbm_gbs": 8 * ncell / (ms * 1e-3) / 1e9,
+                             "roofline_frac": 8 * ncell / (ms * 1e-3) / 1e9 / peak,
+                             "all_interface_kappa_finite": bool(torch.isfinite(kaps[0]).all()),
+                             "minus_kappa_R_mean": float(kk.mean()), "generator_s": gen_s}
+            del phis, kaps, workL, big
 
     # ---- the headline variant and the blank stream once more after an idle gap: the clocks recover from
     # the power cap, which is the regime MEASURED_PEAKS.json's burst figure was taken in (reported beside
@@ -887,6 +918,7 @@ def run_ours(args):
             "stream_ceiling_ms": round(stream_ceiling["ms_per_step"], 4),
             "plic_volume_ms": round(methods["plic_volume"]["ms_per_step"], 4),
             "curvature_ms": None if curv is None else round(curv["ms_per_call"], 4),
+            "curvature_400x400x340_ms": None if curv is None or "large" not in curv else round(curv["large"]["ms_per_call"], 4),
             "storage_ms": None if storage is None else {k: round(v["ms_per_step"], 4) for k, v in storage.items()},
         }
         detail_path = write_detail(line, args.detail_out)
@@ -1004,6 +1036,8 @@ def main(argv=None):
     ap.add_argument("--prewarm-ms", type=float, default=300.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-curvature", action="store_true", help="skip the plic_curvature leg")
+    ap.add_argument("--no-curvature-large", action="store_true",
+                    help="skip the 400 x 400 x 340 lattice of the curvature leg (the paper's raindrop size)")
     ap.add_argument("--no-divergence", action="store_true", help="skip the configs[2] (case-stratified) leg")
     ap.add_argument("--no-config4", action="store_true", help="skip the configs[3] (2^28 snapped/Beta) leg")
     ap.add_argument("--config4-log2n", type=int, default=28)
