@@ -298,7 +298,7 @@ const char *plic_error_string(int code);
 
 /* ABI version: 100*major + minor (1.04: + plic_roundtrip_error, plic_sphere_*, plic_curvature,
  * PLIC_METHOD_KAWANO; 1.05: + plic_solve_h, plic_volume_h, plic_solve_f64, PLIC_METHOD_BLANK in
- * plic_solve). */
+ * plic_solve; 1.06: + plic_curvature_static, PLIC_ERR_CAPACITY). */
 int plic_version(void);
 
 /*

@@ -28,7 +28,7 @@
 #include "plic_curvature.cuh"
 #include "plic_probe.cuh"
 
-#define PLIC_VERSION 105
+#define PLIC_VERSION 106
 
 namespace plic {
 

@@ -47,14 +47,14 @@ def test_header_compiles_as_plain_c(tmp_path):
 
 
 def test_version_and_names(plic):
-    assert plic.plic_version() == 105
+    assert plic.plic_version() == 106
     assert [plic.plic_method_name(i) for i in range(4)] == ["analytic", "sz", "newton", "nested"]
     assert plic.plic_method_name(2 | plic.FAST) == "newton-fast"
     assert plic.plic_method_name(4) == "kawano" and plic.plic_method_name(4 | plic.FAST) is None
     assert plic.plic_method_name(5) is None and plic.plic_method_name(-1) is None
     assert plic.plic_method_name(plic.BLANK) == "blank"
     assert plic.plic_error_string(0) == "ok"
-    for code in (-1, -2, -3, -4, -5):
+    for code in (-1, -2, -3, -4, -5, -6):
         assert plic.plic_error_string(code) not in ("ok", "unknown error code")
 
 
